@@ -1,0 +1,150 @@
+/*
+ * bkr.h -- C ABI of libbkr: block-Krylov (blockCGrQ) solver for the even-odd preconditioned
+ * improved-staggered normal operator M = 4 m^2 - D_eo D_oe on one NVIDIA B200 (sm_100a).
+ *
+ * The calls follow the paper's statement of the problem (arXiv:1710.09745; citations are
+ * "PAPER.md:<line>" of the paper text): one matrix M fixed by the gauge links and the mass,
+ * many right-hand sides, "solve M x = b" (eq. 1), BLOCKCGRQ(X, B) taking an
+ * initial X and the block B (Algorithm 1), relative-residual tolerances
+ * (PAPER.md:322), and the three kernel families the paper optimises: the multi-rhs stencil
+ * (PAPER.md:218-232), streaming multi-BLAS (eq. 3) and reduction multi-BLAS
+ * (eq. 4).
+ *
+ * Conventions
+ *  - Every call returns an int status (BKR_OK = 0, negative = error); nothing throws or exits.
+ *  - Unless a parameter says HOST, pointers are DEVICE pointers owned by the caller (e.g. PyTorch
+ *    allocations); the library never frees or keeps them beyond the call (bkr_load_links copies).
+ *  - Work is enqueued on the CUDA stream given to bkr_create.  Kernel-level calls (pack, dslash,
+ *    apply_M, gram, block_axpy, small-matrix calls) are asynchronous; the solve calls synchronise
+ *    that stream before returning because they report iteration counts.
+ *  - complex = (re, im) pairs.  "canonical" arrays are fp64; "native" arrays are fp64 or fp32.
+ *  - All lattice extents must be even and >= 4 (at extent 4, x+3 wraps onto x-1: legal).
+ *  - 1 <= N <= BKR_MAX_N right-hand sides; anything else -> BKR_EINVAL.
+ *
+ * Layouts
+ *  canonical links   U[mu][s][a][b]      mu = 0..3 (x,y,z,t); s = x + X(y + Y(z + Z t)); 3x3 row-major.
+ *                                        Staggered phases, boundary signs and coefficients are already
+ *                                        multiplied in; backward hops use U(x - h mu)^dagger (eq. 2).
+ *  canonical vector  v[rhs][e][a]        e = s div 2 = even-odd index of a site of the field's parity,
+ *                                        a = colour 0..2; a parity field has Vh = XYZT/2 sites.
+ *  native block      v[e][a][rhs]        the L x N "composite field" of PAPER.md:176, 212-216 stored
+ *                                        row-major (row k = 3 e + a, L = 3 Vh; the N rhs of one row are
+ *                                        contiguous).  bkr_field_bytes() bytes, 256-byte aligned base.
+ *  small matrices    a[i][j]             N x N complex fp64, row-major, device memory.
+ */
+#ifndef BKR_H
+#define BKR_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BKR_MAX_N 32
+
+typedef struct bkr_ctx bkr_ctx; /* opaque: device copies of the links, workspaces, stream */
+
+enum { BKR_F64 = 0, BKR_F32 = 1 };
+
+enum {
+    BKR_OK = 0,
+    BKR_EINVAL = -1,     /* bad argument (dims, N, precision, null pointer, aliasing)             */
+    BKR_ENOLINKS = -2,   /* operator call before bkr_load_links (or fp32 links not requested)      */
+    BKR_ENOMEM = -3,     /* device or host allocation failed                                       */
+    BKR_ECUDA = -4,      /* a CUDA call failed; bkr_last_cuda_error() gives the cudaError_t        */
+    BKR_EBREAKDOWN = -5, /* non-positive / non-finite Cholesky pivot; X = best so far */
+    BKR_ENOCONV = -6     /* maxiter reached; X holds the last iterate, stats are filled             */
+};
+
+typedef struct {
+    int iters;              /* applications of M to the block inside the loop (Alg. 1 l.9)  */
+    int reliable_updates;   /* Algorithm 3 invocations (0 for a pure fp64 solve)            */
+    int status;             /* same value the call returned                                  */
+    int restarts;           /* times the loop was re-entered because the true residual missed tol */
+    double seconds;         /* wall time of the solve loop on the stream (CUDA events)      */
+    double true_relres_max; /* max_i ||b_i - M x_i|| / ||b_i||, recomputed in fp64          */
+    double iter_relres_max; /* max_i ||C[:,i]|| / ||b_i|| the loop stopped on */
+    long long gpu_launches; /* kernels launched by this call                                  */
+} bkr_stats;
+
+/* Create a context for an X*Y*Z*T lattice on CUDA device `device`; `cuda_stream` is a cudaStream_t
+ * (NULL = the legacy default stream).  */
+int bkr_create(bkr_ctx **out, const int dims[4], int device, void *cuda_stream);
+int bkr_destroy(bkr_ctx *ctx);
+
+/* Copy the caller's canonical fat (one-hop) and long (three-hop) links into the library's device
+ * layout (eq. 2; "reordering the ... link fields to achieve memory
+ * coalescing").  also_f32 != 0 additionally keeps an fp32 copy for the inner operator of the
+ * mixed-precision solver.  The caller may free its buffers on return. */
+int bkr_load_links(bkr_ctx *ctx, const void *fat, const void *lng, int also_f32);
+
+/* Bytes of one native block of N rhs on one parity in precision prec (0 on bad arguments). */
+size_t bkr_field_bytes(const bkr_ctx *ctx, int N, int prec);
+
+/* canonical fp64 [rhs][e][a]  <->  native [e][a][rhs] in precision prec. */
+int bkr_pack(bkr_ctx *ctx, int N, int prec, const void *canonical, void *native);
+int bkr_unpack(bkr_ctx *ctx, int N, int prec, const void *native, void *canonical);
+
+/* Multi-rhs stencil: out = D_{out_parity, 1-out_parity} in for all N rhs, each link
+ * matrix loaded once per site and reused for the N vectors.  in/out native, in != out.
+ * out_parity 1: odd <- even (D_oe); 0: even <- odd (D_eo). */
+int bkr_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out);
+
+/* out = 4 m^2 in - D_eo (D_oe in) on even sites ("Schur decomposed"); in/out native. */
+int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out);
+
+/* Reduction multi-BLAS (eq. 4): K = X^dag Y, k_ij = sum_k conj(x_ki) y_kj, one pass over
+ * the blocks, fp64 accumulation, deterministic two-stage reduction.  hermitian != 0: only i <= j is
+ * computed and the rest mirrored with a real diagonal.  X, Y native; K N*N complex fp64. */
+int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, void *K);
+
+/* Streaming multi-BLAS (eq. 3): Y <- Y + X a, y_kj += sum_i x_ki a_ij, every vector
+ * streamed once.  a: N*N complex fp64; X, Y native, X != Y. */
+int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y);
+
+/* Small dense algebra on the device, one warp (Algorithm 2 l.3):
+ * bkr_cholesky_upper: H = R^dag R, R upper triangular with real positive diagonal; Rinv = R^-1.
+ * bkr_hpd_inverse   : Ginv = G^-1 for Hermitian positive-definite G (via Cholesky).
+ * Inputs use the upper triangle only.  status (device int, may be NULL) receives BKR_OK/BKR_EBREAKDOWN. */
+int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, int *status);
+int bkr_hpd_inverse(bkr_ctx *ctx, int N, const void *G, void *Ginv, int *status);
+
+/* blockCGrQ (Algorithm 1) for M X = B, N rhs on even sites.
+ * B, X: canonical fp64 device arrays; X holds the initial guess on entry and the solution on return.
+ * Stops when max_i ||r_i|| / ||b_i|| <= tol (iterated residual from C), then recomputes the
+ * true residual in fp64 and, if it misses tol, re-enters the loop from X (counted in stats->restarts).
+ * inner_prec = BKR_F64: pure fp64.  BKR_F32: P, Q, MP and the inner operator in fp32 with block reliable
+ * updates (Algorithm 3) whenever the max relative residual dropped by `delta`.
+ * true_relres: HOST array of N doubles (may be NULL).  stats: HOST (may be NULL). */
+int bkr_solve_block(bkr_ctx *ctx, double mass, int N, const void *B, void *X, double tol, int maxiter,
+                    int inner_prec, double delta, double *true_relres, bkr_stats *stats);
+
+/* The paper's baseline: CG on each rhs.  batched = 0: N sequential single-rhs solves;
+ * batched = 1: one CG loop sharing the multi-rhs stencil with per-rhs scalars ("pseudo-block",
+ * PAPER.md:77).  iters: HOST array of N ints (may be NULL). */
+int bkr_solve_cg(bkr_ctx *ctx, double mass, int N, const void *B, void *X, double tol, int maxiter,
+                 int batched, int *iters, double *true_relres, bkr_stats *stats);
+
+/* End-to-end variants: B and X are HOST arrays (canonical fp64); the host->device copy of B and X0 and
+ * the device->host copy of X run inside the call. */
+int bkr_solve_block_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void *X_host, double tol,
+                         int maxiter, int inner_prec, double delta, double *true_relres, bkr_stats *stats);
+int bkr_solve_cg_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void *X_host, double tol,
+                      int maxiter, int batched, int *iters, double *true_relres, bkr_stats *stats);
+
+/* One full blockCGrQ iteration (Alg. 1 l.8-12) on synthetic state, for benchmarking the hot path
+ * without a solve: initialises Q, P, C from B (canonical fp64) on the first call for this N/prec and
+ * then enqueues `iters` iterations (no convergence test, no host sync).  Returns kernels launched
+ * in *launches (HOST, may be NULL). */
+int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void *B, int iters,
+                         long long *launches);
+
+int bkr_last_cuda_error(const bkr_ctx *ctx);
+const char *bkr_strerror(int status);
+const char *bkr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BKR_H */

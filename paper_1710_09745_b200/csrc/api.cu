@@ -1,0 +1,245 @@
+// C ABI of libbkr (include/bkr.h): argument checking and dispatch only; all arithmetic is in the kernels.
+#include "common.cuh"
+
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+static bool valid_n(int N) { return N >= 1 && N <= BKR_MAX_N; }
+static bool valid_prec(int p) { return p == BKR_F64 || p == BKR_F32; }
+
+extern "C" {
+
+int bkr_create(bkr_ctx **out, const int dims[4], int device, void *cuda_stream)
+{
+    if (!out || !dims) return BKR_EINVAL;
+    *out = nullptr;
+    long long V = 1;
+    for (int mu = 0; mu < 4; mu++) {
+        if (dims[mu] < 4 || (dims[mu] & 1)) return BKR_EINVAL;
+        V *= dims[mu];
+    }
+    if (V > (1LL << 30)) return BKR_EINVAL; // site indices are 32-bit; element offsets are 64-bit
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return BKR_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return BKR_ECUDA;
+    bkr_ctx *ctx = (bkr_ctx *)calloc(1, sizeof(bkr_ctx));
+    if (!ctx) return BKR_ENOMEM;
+    for (int mu = 0; mu < 4; mu++) ctx->g.X[mu] = dims[mu];
+    ctx->g.V = (int)V;
+    ctx->g.Vh = (int)(V / 2);
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    if (cudaMalloc((void **)&ctx->small, (size_t)4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)) != cudaSuccess) {
+        free(ctx);
+        return BKR_ENOMEM;
+    }
+    *out = ctx;
+    return BKR_OK;
+}
+
+int bkr_destroy(bkr_ctx *ctx)
+{
+    if (!ctx) return BKR_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    solver_free_workspace(ctx);
+    cudaFree(ctx->links64);
+    cudaFree(ctx->links32);
+    cudaFree(ctx->tmp_odd[0]);
+    cudaFree(ctx->tmp_odd[1]);
+    cudaFree(ctx->partials);
+    cudaFree(ctx->small);
+    free(ctx);
+    return BKR_OK;
+}
+
+int bkr_load_links(bkr_ctx *ctx, const void *fat, const void *lng, int also_f32)
+{
+    if (!ctx || !fat || !lng) return BKR_EINVAL;
+    size_t n = (size_t)2 * 4 * ctx->g.V * 9;
+    if (!ctx->links64) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->links64, n * sizeof(double2)));
+    if (also_f32 && !ctx->links32) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->links32, n * sizeof(float2)));
+    return launch_pack_links(ctx, (const double2 *)fat, (const double2 *)lng, ctx->links64,
+                             also_f32 ? ctx->links32 : nullptr);
+}
+
+size_t bkr_field_bytes(const bkr_ctx *ctx, int N, int prec)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec)) return 0;
+    return field_elems(ctx->g, N) * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
+}
+
+int bkr_pack(bkr_ctx *ctx, int N, int prec, const void *canonical, void *native)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !canonical || !native || canonical == native) return BKR_EINVAL;
+    return launch_pack(ctx, N, prec, (const double2 *)canonical, native);
+}
+
+int bkr_unpack(bkr_ctx *ctx, int N, int prec, const void *native, void *canonical)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !canonical || !native || canonical == native) return BKR_EINVAL;
+    return launch_unpack(ctx, N, prec, native, (double2 *)canonical);
+}
+
+int bkr_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !in || !out || in == out) return BKR_EINVAL;
+    if (out_parity != 0 && out_parity != 1) return BKR_EINVAL;
+    return launch_dslash(ctx, out_parity, N, prec, in, out, nullptr, 0.0, nullptr);
+}
+
+int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !in || !out || in == out) return BKR_EINVAL;
+    if (!(prec == BKR_F64 ? (void *)ctx->links64 : (void *)ctx->links32)) return BKR_ENOLINKS;
+    BKR_TRY(ensure_tmp_odd(ctx, N, prec));
+    BKR_TRY(launch_dslash(ctx, 1, N, prec, in, ctx->tmp_odd[prec], nullptr, 0.0, nullptr));
+    return launch_dslash(ctx, 0, N, prec, ctx->tmp_odd[prec], out, in, 4.0 * mass * mass, nullptr);
+}
+
+int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, void *K)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !X || !Y || !K) return BKR_EINVAL;
+    int np = 0;
+    BKR_TRY(launch_gram_partials(ctx, N, prec, X, Y, hermitian ? 1 : 0, &np, nullptr));
+    return launch_gram_finish(ctx, N, np, hermitian ? 1 : 0, (double2 *)K);
+}
+
+int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !a || !X || !Y || X == Y) return BKR_EINVAL;
+    return launch_block_update(ctx, N, prec, prec, (const double2 *)a, Y, X, Y, nullptr);
+}
+
+int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, int *status)
+{
+    if (!ctx || !valid_n(N) || !H || !R) return BKR_EINVAL;
+    SmallArgs a;
+    memset(&a, 0, sizeof(a));
+    a.N = N;
+    a.mode = SMALL_CHOL;
+    a.in = (const double2 *)H;
+    a.out0 = (double2 *)R;
+    a.out1 = (double2 *)Rinv;
+    a.status = status;
+    return launch_small(ctx, a);
+}
+
+int bkr_hpd_inverse(bkr_ctx *ctx, int N, const void *G, void *Ginv, int *status)
+{
+    if (!ctx || !valid_n(N) || !G || !Ginv) return BKR_EINVAL;
+    SmallArgs a;
+    memset(&a, 0, sizeof(a));
+    a.N = N;
+    a.mode = SMALL_HPDINV;
+    a.in = (const double2 *)G;
+    a.out0 = (double2 *)Ginv;
+    a.status = status;
+    return launch_small(ctx, a);
+}
+
+static bool valid_solve(bkr_ctx *ctx, int N, const void *B, void *X, double tol, int maxiter)
+{
+    return ctx && valid_n(N) && B && X && B != X && tol > 0.0 && maxiter >= 0;
+}
+
+int bkr_solve_block(bkr_ctx *ctx, double mass, int N, const void *B, void *X, double tol, int maxiter, int inner_prec,
+                    double delta, double *true_relres, bkr_stats *stats)
+{
+    if (!valid_solve(ctx, N, B, X, tol, maxiter) || !valid_prec(inner_prec)) return BKR_EINVAL;
+    if (inner_prec == BKR_F32 && !(delta > 0.0 && delta < 1.0)) return BKR_EINVAL;
+    if (!ctx->links64 || (inner_prec == BKR_F32 && !ctx->links32)) return BKR_ENOLINKS;
+    int rc = solver_block(ctx, mass, N, (const double2 *)B, (double2 *)X, tol, maxiter, inner_prec, delta, true_relres,
+                          stats);
+    if (stats) stats->status = rc;
+    return rc;
+}
+
+int bkr_solve_cg(bkr_ctx *ctx, double mass, int N, const void *B, void *X, double tol, int maxiter, int batched,
+                 int *iters, double *true_relres, bkr_stats *stats)
+{
+    if (!valid_solve(ctx, N, B, X, tol, maxiter)) return BKR_EINVAL;
+    if (!ctx->links64) return BKR_ENOLINKS;
+    int rc = solver_cg(ctx, mass, N, (const double2 *)B, (double2 *)X, tol, maxiter, batched ? 1 : 0, iters,
+                       true_relres, stats);
+    if (stats) stats->status = rc;
+    return rc;
+}
+
+// host-buffer variants: staging through two device blocks owned by the call
+static int with_host_buffers(bkr_ctx *ctx, int N, const void *B_host, void *X_host, double2 **dB, double2 **dX)
+{
+    size_t bytes = field_elems(ctx->g, N) * sizeof(double2);
+    *dB = *dX = nullptr;
+    BKR_CUDA(ctx, cudaMalloc((void **)dB, bytes));
+    if (cudaMalloc((void **)dX, bytes) != cudaSuccess) {
+        cudaFree(*dB);
+        *dB = nullptr;
+        return BKR_ENOMEM;
+    }
+    BKR_CUDA(ctx, cudaMemcpyAsync(*dB, B_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    BKR_CUDA(ctx, cudaMemcpyAsync(*dX, X_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
+    return BKR_OK;
+}
+
+static int finish_host_buffers(bkr_ctx *ctx, int N, void *X_host, double2 *dB, double2 *dX, int rc)
+{
+    size_t bytes = field_elems(ctx->g, N) * sizeof(double2);
+    cudaError_t e = cudaMemcpyAsync(X_host, dX, bytes, cudaMemcpyDeviceToHost, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(dB);
+    cudaFree(dX);
+    if (e != cudaSuccess) {
+        ctx->last_cuda = (int)e;
+        return BKR_ECUDA;
+    }
+    return rc;
+}
+
+int bkr_solve_block_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void *X_host, double tol, int maxiter,
+                         int inner_prec, double delta, double *true_relres, bkr_stats *stats)
+{
+    if (!valid_solve(ctx, N, B_host, X_host, tol, maxiter)) return BKR_EINVAL;
+    double2 *dB, *dX;
+    BKR_TRY(with_host_buffers(ctx, N, B_host, X_host, &dB, &dX));
+    int rc = bkr_solve_block(ctx, mass, N, dB, dX, tol, maxiter, inner_prec, delta, true_relres, stats);
+    return finish_host_buffers(ctx, N, X_host, dB, dX, rc);
+}
+
+int bkr_solve_cg_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void *X_host, double tol, int maxiter,
+                      int batched, int *iters, double *true_relres, bkr_stats *stats)
+{
+    if (!valid_solve(ctx, N, B_host, X_host, tol, maxiter)) return BKR_EINVAL;
+    double2 *dB, *dX;
+    BKR_TRY(with_host_buffers(ctx, N, B_host, X_host, &dB, &dX));
+    int rc = bkr_solve_cg(ctx, mass, N, dB, dX, tol, maxiter, batched, iters, true_relres, stats);
+    return finish_host_buffers(ctx, N, X_host, dB, dX, rc);
+}
+
+int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void *B, int iters, long long *launches)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !B || iters < 0) return BKR_EINVAL;
+    if (!ctx->links64 || (prec == BKR_F32 && !ctx->links32)) return BKR_ENOLINKS;
+    return solver_bench_iterations(ctx, mass, N, prec, (const double2 *)B, iters, launches);
+}
+
+int bkr_last_cuda_error(const bkr_ctx *ctx) { return ctx ? ctx->last_cuda : 0; }
+
+const char *bkr_strerror(int status)
+{
+    switch (status) {
+    case BKR_OK: return "ok";
+    case BKR_EINVAL: return "invalid argument";
+    case BKR_ENOLINKS: return "links not loaded (or no fp32 copy requested)";
+    case BKR_ENOMEM: return "out of memory";
+    case BKR_ECUDA: return "CUDA error (see bkr_last_cuda_error)";
+    case BKR_EBREAKDOWN: return "Cholesky breakdown: block lost rank or non-finite Gram matrix";
+    case BKR_ENOCONV: return "maxiter reached without convergence";
+    default: return "unknown status";
+    }
+}
+
+const char *bkr_version(void) { return "libbkr 0.1 (sm_100a)"; }
+
+} // extern "C"

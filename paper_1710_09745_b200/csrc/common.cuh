@@ -1,0 +1,149 @@
+// Internal declarations of libbkr (sm_100a).  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/bkr.h"
+
+#define BKR_NUM_SMS 148 /* B200: 2 dies x 74 SMs; grids are sized in multiples of this */
+
+struct Geom {
+    int X[4];     // extents x,y,z,t (all even, >= 4)
+    int V, Vh;    // sites, sites per parity (48^3 x 96 = 10.6 M fits an int)
+};
+
+template <typename Real> struct CxT;
+template <> struct CxT<double> { typedef double2 type; };
+template <> struct CxT<float> { typedef float2 type; };
+
+// Flags the solver kernels share (device memory).  Every loop kernel returns at once when done != 0,
+// so the host can enqueue iterations in batches without synchronising.
+struct SolverFlags {
+    int done;          // 1: converged or broken down -> loop kernels become no-ops
+    int breakdown;     // 1: non-positive / non-finite Cholesky pivot
+    int iters;         // completed iterations (Alg. 1 l.9 applications of M)
+    int want_update;   // mixed precision: reliable update requested (Alg. 3)
+    double relres_max; // max_i ||C[:,i]|| / ||b_i||  after the last l.12
+    double relres_last_update;
+};
+
+struct bkr_ctx {
+    Geom g;
+    int device;
+    cudaStream_t stream;
+    int last_cuda;
+    long long launches;
+    // links in the device layout L[((type*4+mu)*2+parity)*9+el][e], type 0 fat / 1 long
+    double2 *links64;
+    float2 *links32;
+    // scratch for apply_M (odd-parity temporary), grown on demand, per precision
+    void *tmp_odd[2];
+    size_t tmp_odd_bytes[2];
+    // two-stage reduction scratch: [num_ctas][N*N] complex fp64
+    double2 *partials;
+    size_t partials_bytes;
+    // small-matrix scratch for the API-level gram / cholesky calls
+    double2 *small;
+    // solver workspace (allocated on first solve for a given N / precision, reused)
+    struct Workspace *ws;
+};
+
+#define BKR_CUDA(ctx, call)                                   \
+    do {                                                      \
+        cudaError_t e_ = (call);                              \
+        if (e_ != cudaSuccess) {                              \
+            (ctx)->last_cuda = (int)e_;                       \
+            return e_ == cudaErrorMemoryAllocation ? BKR_ENOMEM : BKR_ECUDA; \
+        }                                                     \
+    } while (0)
+
+#define BKR_TRY(call)                 \
+    do {                              \
+        int rc_ = (call);             \
+        if (rc_ != BKR_OK) return rc_; \
+    } while (0)
+
+static inline int bkr_check_launch(bkr_ctx *ctx)
+{
+    cudaError_t e = cudaGetLastError();
+    ctx->launches++;
+    if (e != cudaSuccess) {
+        ctx->last_cuda = (int)e;
+        return BKR_ECUDA;
+    }
+    return BKR_OK;
+}
+
+static inline size_t field_elems(const Geom &g, int N) { return (size_t)g.Vh * 3 * (size_t)N; }
+
+// ---- layout.cu
+int launch_pack_links(bkr_ctx *ctx, const double2 *fat, const double2 *lng, double2 *out64, float2 *out32);
+int launch_pack(bkr_ctx *ctx, int N, int prec, const double2 *canonical, void *native);
+int launch_unpack(bkr_ctx *ctx, int N, int prec, const void *native, double2 *canonical);
+int launch_convert(bkr_ctx *ctx, size_t n_complex, int src_prec, const void *src, int dst_prec, void *dst,
+                   const int *done);
+
+// ---- dslash.cu :  out = D in   or (xpay) out = a * xp - D in
+int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp,
+                  double a, const int *done);
+
+// ---- blas.cu
+// stage 1 of K = X^dag Y: per-CTA partial sums into ctx->partials; returns the number of partials.
+int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian,
+                         int *num_partials, const int *done);
+// stage 2 alone (API path): K = fixed-order sum of the partials, mirrored if hermitian.
+int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K);
+// Z = C + W a   (C may be NULL = 0; Z may alias C; Z must not alias W).  a: N x N complex fp64 (device).
+// precZ is the precision of Z and C, precW of W; arithmetic in precZ.
+int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C,
+                        const void *W, void *Z, const int *done);
+// per-column reductions (two-stage, deterministic), results in out[j], j < N (device fp64):
+//   mode 0: sum_k |x_kj|^2        mode 1: Re sum_k conj(x_kj) y_kj      mode 2: sum_k |x_kj - y_kj|^2
+int launch_col_reduce(bkr_ctx *ctx, int N, int prec, int mode, const void *X, const void *Y, double *out,
+                      const int *done);
+// Z = alpha * X + beta * Y elementwise with per-call real scalars (Y may be NULL); all precision prec.
+int launch_axpby(bkr_ctx *ctx, size_t n_complex, int prec, double alpha, const void *X, double beta,
+                 const void *Y, void *Z, const int *done);
+// batched CG updates with per-column real coefficients coef[j] (device fp64):
+//   mode 0: X += coef * P ; R -= coef * Q        mode 1: P = R + coef * P
+int launch_cg_update(bkr_ctx *ctx, int N, int prec, int mode, const double *coef, void *X, const void *P,
+                     void *R, const void *Q, const int *done);
+
+// ---- small.cu : one-CTA kernels for the N x N algebra, see small.cu for the modes
+struct SmallArgs {
+    int N;
+    int mode;
+    int num_partials;        // > 0: input matrix = fixed-order sum of ctx partials; 0: read `in`
+    const double2 *partials; // [num_partials][N*N]
+    const double2 *in;       // N x N (upper triangle used)
+    double2 *C, *Cprev, *Cinv; // residual factor (Alg. 1 l.4, l.12), its previous value, its inverse
+    double2 *negbeta, *W;    // -beta and W = beta C  (Alg. 1 l.9, l.10)
+    double2 *Sinv, *Sdag;    // S^-1 and S^dagger (Alg. 1 l.11 / l.8)
+    double2 *out0, *out1;    // API path outputs
+    const double *bnorm;     // ||b_i||
+    double tol, delta;
+    SolverFlags *flags;
+    int *status;             // API path
+    int mixed;
+};
+enum { SMALL_CHOL = 0, SMALL_HPDINV = 1, SMALL_BETA = 2, SMALL_QR = 3, SMALL_INIT = 4, SMALL_RELUPD = 5 };
+int launch_small(bkr_ctx *ctx, const SmallArgs &args);
+// CG scalar kernel: per-rhs alpha / beta / convergence bookkeeping
+struct CgScalars {
+    double rho[BKR_MAX_N], pAp[BKR_MAX_N], rho_new[BKR_MAX_N], bb[BKR_MAX_N];
+    double alpha[BKR_MAX_N], beta[BKR_MAX_N];
+    int iters[BKR_MAX_N], conv[BKR_MAX_N];
+};
+int launch_cg_scalar(bkr_ctx *ctx, int N, int step, double tol, CgScalars *s, SolverFlags *flags);
+
+// ---- solver.cu
+int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, double tol, int maxiter,
+                 int inner_prec, double delta, double *true_relres, bkr_stats *stats);
+int solver_cg(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, double tol, int maxiter,
+              int batched, int *iters, double *true_relres, bkr_stats *stats);
+int solver_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const double2 *B, int iters,
+                            long long *launches);
+void solver_free_workspace(bkr_ctx *ctx);
+int ensure_partials(bkr_ctx *ctx, size_t bytes);
+int ensure_tmp_odd(bkr_ctx *ctx, int N, int prec);

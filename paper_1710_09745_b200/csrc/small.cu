@@ -1,0 +1,325 @@
+// Small dense N x N algebra on the device (PAPER.md:178 does it on the host with Eigen; north_star moves it
+// into a device-side kernel so that no Gram matrix or coefficient matrix ever crosses to the host).
+//
+// One CTA.  All threads: the deterministic second stage of the Gram reduction (fixed-order sum of the per-CTA
+// partials, Hermitised from the upper triangle) and the N x N products.  Warp 0 alone: the
+// Cholesky factorisation H = R^dag R (Algorithm 2 l.3) and the triangular inverse, matrices in shared memory.
+//
+// Modes (Algorithm 1 / 2 / 3 line numbers as reconstructed in DESIGN.md U7):
+//   SMALL_CHOL    API: R = chol(in), Rinv
+//   SMALL_HPDINV  API: out0 = in^-1
+//   SMALL_BETA    l.9/l.10: G = sum partials; beta = G^-1; negbeta = -beta; W = beta C
+//   SMALL_QR      l.11/l.12: H = sum partials; S = chol(H); Sinv; Sdag; Cprev = C; C = S C; residuals, flags
+//   SMALL_INIT    l.4-l.5:  H = sum partials; C = chol(H); Sinv = C^-1 (to form Q = R C^-1); Sdag = 1
+//   SMALL_RELUPD  Alg. 3 l.5-l.6: C_new = chol(H); Sinv = C_new^-1; Sdag = (C_new Cprev^-1)^dag; C = C_new
+#include "common.cuh"
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b)
+{
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}
+__device__ __forceinline__ double2 cmulc(double2 a, double2 b) // conj(a) * b
+{
+    return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+}
+
+// In-place upper Cholesky of the Hermitian matrix whose upper triangle is in A (row-major, shared memory).
+// On return A = R (upper triangular, real positive diagonal, zeros below).  One warp; lane = column.
+__device__ bool warp_cholesky_upper(int N, double2 *A, int lane)
+{
+    for (int j = 0; j < N; j++) {
+        double d = A[j * N + j].x;
+        if (!(d > 0.0) || !isfinite(d)) return false; // uniform across the warp
+        double rjj = sqrt(d);
+        __syncwarp();
+        if (lane < N) {
+            if (lane == j) A[j * N + j] = make_double2(rjj, 0.0);
+            else if (lane > j) {
+                double2 v = A[j * N + lane];
+                A[j * N + lane] = make_double2(v.x / rjj, v.y / rjj);
+            } else A[j * N + lane] = make_double2(0.0, 0.0);
+        }
+        __syncwarp();
+        if (lane > j && lane < N) {
+            double2 rjc = A[j * N + lane];
+            for (int i = j + 1; i <= lane; i++) {
+                double2 t = cmulc(A[j * N + i], rjc);
+                double2 v = A[i * N + lane];
+                A[i * N + lane] = make_double2(v.x - t.x, v.y - t.y);
+            }
+        }
+        __syncwarp();
+    }
+    return true;
+}
+
+// Ri = R^-1 for upper-triangular R with real diagonal; lane = column of Ri (back substitution).
+__device__ void warp_upper_inverse(int N, const double2 *R, double2 *Ri, int lane)
+{
+    if (lane < N) {
+        int c = lane;
+        for (int i = N - 1; i > c; i--) Ri[i * N + c] = make_double2(0.0, 0.0);
+        Ri[c * N + c] = make_double2(1.0 / R[c * N + c].x, 0.0);
+        for (int i = c - 1; i >= 0; i--) {
+            double2 s = make_double2(0.0, 0.0);
+            for (int k = i + 1; k <= c; k++) {
+                double2 t = cmul(R[i * N + k], Ri[k * N + c]);
+                s.x += t.x;
+                s.y += t.y;
+            }
+            double d = R[i * N + i].x;
+            Ri[i * N + c] = make_double2(-s.x / d, -s.y / d);
+        }
+    }
+    __syncwarp();
+}
+
+__device__ void load_hermitian(const SmallArgs &p, double2 *A)
+{
+    const int N = p.N;
+    for (int o = threadIdx.x; o < N * N; o += blockDim.x) {
+        int i = o / N, j = o % N;
+        int src = i <= j ? o : j * N + i;
+        double2 s = make_double2(0.0, 0.0);
+        if (p.num_partials > 0) {
+            for (int q = 0; q < p.num_partials; q++) { // fixed order: deterministic
+                double2 v = p.partials[(size_t)q * N * N + src];
+                s.x += v.x;
+                s.y += v.y;
+            }
+        } else s = p.in[src];
+        if (i > j) s.y = -s.y;
+        if (i == j) s.y = 0.0;
+        A[o] = s;
+    }
+    __syncthreads();
+}
+
+// residual norms from C (PAPER.md:208 with the index fix U11): r_i = ||C[:,i]|| / ||b_i||
+__device__ double max_relres(int N, const double2 *C, const double *bnorm, double *scratch)
+{
+    for (int i = threadIdx.x; i < N; i += blockDim.x) {
+        double s = 0.0;
+        for (int j = 0; j < N; j++) {
+            double2 v = C[j * N + i];
+            s += v.x * v.x + v.y * v.y;
+        }
+        scratch[i] = sqrt(s) / bnorm[i];
+    }
+    __syncthreads();
+    double m = 0.0;
+    for (int i = 0; i < N; i++) m = fmax(m, scratch[i]);
+    __syncthreads();
+    return m;
+}
+
+__global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
+{
+    extern __shared__ double2 sm[];
+    const int N = p.N, NN = N * N;
+    double2 *A = sm, *B = sm + NN, *Cm = sm + 2 * NN, *Dm = sm + 3 * NN;
+    __shared__ int ok_s;
+    __shared__ double scratch[BKR_MAX_N];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    SolverFlags *fl = p.flags;
+    if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) return;
+
+    load_hermitian(p, A);
+    if (warp == 0) {
+        bool ok = warp_cholesky_upper(N, A, lane); // A = R
+        if (ok) warp_upper_inverse(N, A, B, lane); // B = R^-1
+        if (lane == 0) ok_s = ok ? 1 : 0;
+    }
+    __syncthreads();
+    const bool ok = ok_s != 0;
+    if (!ok) {
+        if (threadIdx.x == 0) {
+            if (p.status) *p.status = BKR_EBREAKDOWN;
+            if (fl) {
+                fl->breakdown = 1;
+                fl->done = 1;
+            }
+        }
+        return;
+    }
+    if (threadIdx.x == 0 && p.status) *p.status = BKR_OK;
+
+    switch (p.mode) {
+    case SMALL_CHOL:
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            p.out0[o] = A[o];
+            if (p.out1) p.out1[o] = B[o];
+        }
+        break;
+    case SMALL_HPDINV:
+    case SMALL_BETA: {
+        // beta = R^-1 R^-dag : beta_ij = sum_k Ri_ik conj(Ri_jk), k >= max(i,j)
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            int i = o / N, j = o % N;
+            double2 s = make_double2(0.0, 0.0);
+            for (int k = (i > j ? i : j); k < N; k++) {
+                double2 t = cmulc(B[j * N + k], B[i * N + k]);
+                s.x += t.x;
+                s.y += t.y;
+            }
+            Cm[o] = s;
+        }
+        __syncthreads();
+        if (p.mode == SMALL_HPDINV) {
+            for (int o = threadIdx.x; o < NN; o += blockDim.x) p.out0[o] = Cm[o];
+            break;
+        }
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            Dm[o] = p.C[o];
+            p.negbeta[o] = make_double2(-Cm[o].x, -Cm[o].y);
+        }
+        __syncthreads();
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) { // W = beta C, C upper triangular
+            int i = o / N, j = o % N;
+            double2 s = make_double2(0.0, 0.0);
+            for (int k = 0; k <= j; k++) {
+                double2 t = cmul(Cm[i * N + k], Dm[k * N + j]);
+                s.x += t.x;
+                s.y += t.y;
+            }
+            p.W[o] = s;
+        }
+        break;
+    }
+    case SMALL_QR: {
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            int i = o / N, j = o % N;
+            double2 c = p.C[o];
+            Dm[o] = c;
+            p.Cprev[o] = c;
+            p.Sinv[o] = B[o];
+            double2 s = A[j * N + i]; // S^dag_ij = conj(S_ji)
+            p.Sdag[o] = make_double2(s.x, -s.y);
+        }
+        __syncthreads();
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) { // C = S C, both upper triangular
+            int i = o / N, j = o % N;
+            double2 s = make_double2(0.0, 0.0);
+            for (int k = i; k <= j; k++) {
+                double2 t = cmul(A[i * N + k], Dm[k * N + j]);
+                s.x += t.x;
+                s.y += t.y;
+            }
+            Cm[o] = s;
+            p.C[o] = s;
+        }
+        __syncthreads();
+        double r = max_relres(N, Cm, p.bnorm, scratch);
+        if (threadIdx.x == 0) {
+            fl->iters += 1;
+            fl->relres_max = r;
+            if (!p.mixed) {
+                if (r <= p.tol) fl->done = 1;
+            } else if (r < p.delta * fl->relres_last_update || r <= p.tol) fl->want_update = 1;
+        }
+        break;
+    }
+    case SMALL_INIT: {
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            int i = o / N, j = o % N;
+            p.C[o] = A[o];
+            p.Cprev[o] = A[o];
+            p.Sinv[o] = B[o];
+            p.Sdag[o] = make_double2(i == j ? 1.0 : 0.0, 0.0);
+        }
+        double r = max_relres(N, A, p.bnorm, scratch);
+        if (threadIdx.x == 0) {
+            fl->relres_max = r;
+            fl->relres_last_update = r;
+            fl->want_update = 0;
+            if (r <= p.tol) fl->done = 1;
+        }
+        break;
+    }
+    case SMALL_RELUPD: {
+        // A = C_new, B = C_new^-1.  S = C_new Cprev^-1 (Alg. 3 l.6, C_old = C before this iteration's l.12: U12)
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) Dm[o] = p.Cprev[o];
+        __syncthreads();
+        if (warp == 0) warp_upper_inverse(N, Dm, Cm, lane); // Cm = Cprev^-1
+        __syncthreads();
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            int i = o / N, j = o % N;
+            double2 s = make_double2(0.0, 0.0);
+            for (int k = i; k <= j; k++) {
+                double2 t = cmul(A[i * N + k], Cm[k * N + j]);
+                s.x += t.x;
+                s.y += t.y;
+            }
+            Dm[o] = s; // S_ij
+        }
+        __syncthreads();
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            int i = o / N, j = o % N;
+            double2 s = Dm[j * N + i];
+            p.Sdag[o] = make_double2(s.x, -s.y);
+            p.Sinv[o] = B[o];
+            p.C[o] = A[o];
+        }
+        double r = max_relres(N, A, p.bnorm, scratch);
+        if (threadIdx.x == 0) {
+            fl->relres_max = r;
+            fl->relres_last_update = r;
+            fl->want_update = 0;
+            if (r <= p.tol) fl->done = 1;
+        }
+        break;
+    }
+    }
+}
+
+int launch_small(bkr_ctx *ctx, const SmallArgs &args)
+{
+    size_t smem = (size_t)4 * args.N * args.N * sizeof(double2);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
+        attr_set = true;
+    }
+    small_kernel<<<1, 256, smem, ctx->stream>>>(args);
+    return bkr_check_launch(ctx);
+}
+
+// Scalars of the CG baseline (ref. [40]): step 0: alpha = rho / pAp; step 1: beta = rho'/rho,
+// convergence per rhs, rho = rho'.  A converged rhs keeps alpha = 0 so that its x no longer changes.
+__global__ void cg_scalar_kernel(int N, int step, double tol, CgScalars *s, SolverFlags *fl)
+{
+    if (fl->done) return;
+    int j = threadIdx.x;
+    __shared__ int all_conv;
+    if (j == 0) all_conv = 1;
+    __syncthreads();
+    if (j < N) {
+        if (step == 2) { // initial residual already below tol?
+            if (sqrt(s->rho[j] / s->bb[j]) <= tol) s->conv[j] = 1;
+            else all_conv = 0;
+        } else if (step == 0) {
+            s->alpha[j] = s->conv[j] ? 0.0 : s->rho[j] / s->pAp[j];
+        } else {
+            if (!s->conv[j]) {
+                s->iters[j] += 1;
+                double rn = s->rho_new[j];
+                s->beta[j] = rn / s->rho[j];
+                s->rho[j] = rn;
+                if (sqrt(rn / s->bb[j]) <= tol) s->conv[j] = 1;
+            } else s->beta[j] = 0.0;
+            if (!s->conv[j]) all_conv = 0;
+        }
+    }
+    __syncthreads();
+    if (j == 0 && step != 0) {
+        if (step == 1) fl->iters += 1;
+        if (all_conv) fl->done = 1;
+    }
+}
+
+int launch_cg_scalar(bkr_ctx *ctx, int N, int step, double tol, CgScalars *s, SolverFlags *flags)
+{
+    cg_scalar_kernel<<<1, 32, 0, ctx->stream>>>(N, step, tol, s, flags);
+    return bkr_check_launch(ctx);
+}

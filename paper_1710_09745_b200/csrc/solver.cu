@@ -1,0 +1,398 @@
+// Host-side drivers: blockCGrQ (Algorithm 1, reconstructed in DESIGN.md U7), block reliable
+// updates (Algorithm 3, U12-U14) and the CG baseline.  The host only enqueues
+// kernels: Gram matrices, coefficient matrices and residual norms stay on the device (small.cu); every loop
+// kernel is a no-op once flags->done is set, so iterations are enqueued in batches and the host looks at the
+// flags once per batch.
+#include "common.cuh"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+struct Workspace {
+    int N, prec;
+    size_t bytes64, bytesP;
+    double2 *Bn, *Xn, *Y, *R64;   // fp64 native blocks (Y, R64 only for the mixed solver; else R64 aliases AP)
+    void *Q, *Q2, *P, *P2, *AP;   // inner-precision native blocks
+    double2 *C, *Cprev, *negbeta, *W, *Sinv, *Sdag;
+    double *bnorm2, *colred;
+    SolverFlags *flags, *h_flags;
+    CgScalars *cgs, *h_cgs;
+    // CG baseline blocks (fp64): r, p, q
+    double2 *cg_r, *cg_p, *cg_q;
+    int cgN;
+    cudaEvent_t ev0, ev1;
+    bool bench_ready;
+};
+
+static void free_ws(Workspace *w)
+{
+    if (!w) return;
+    cudaFree(w->Bn); cudaFree(w->Xn); cudaFree(w->Y);
+    if (w->prec != BKR_F64) cudaFree(w->R64);
+    cudaFree(w->Q); cudaFree(w->Q2); cudaFree(w->P); cudaFree(w->P2); cudaFree(w->AP);
+    cudaFree(w->C); cudaFree(w->bnorm2); cudaFree(w->flags); cudaFree(w->cgs);
+    cudaFree(w->cg_r); cudaFree(w->cg_p); cudaFree(w->cg_q);
+    cudaFreeHost(w->h_flags); cudaFreeHost(w->h_cgs);
+    if (w->ev0) cudaEventDestroy(w->ev0);
+    if (w->ev1) cudaEventDestroy(w->ev1);
+    free(w);
+}
+
+void solver_free_workspace(bkr_ctx *ctx)
+{
+    free_ws(ctx->ws);
+    ctx->ws = nullptr;
+}
+
+int ensure_tmp_odd(bkr_ctx *ctx, int N, int prec)
+{
+    size_t need = field_elems(ctx->g, N) * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
+    if (ctx->tmp_odd_bytes[prec] >= need) return BKR_OK;
+    if (ctx->tmp_odd[prec]) cudaFree(ctx->tmp_odd[prec]);
+    ctx->tmp_odd[prec] = nullptr;
+    ctx->tmp_odd_bytes[prec] = 0;
+    BKR_CUDA(ctx, cudaMalloc(&ctx->tmp_odd[prec], need));
+    ctx->tmp_odd_bytes[prec] = need;
+    return BKR_OK;
+}
+
+// common small allocations; blocks are allocated by the block / CG entry points as they need them
+static int get_ws(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fields)
+{
+    Workspace *w = ctx->ws;
+    if (w && (w->N != N || w->prec != prec)) {
+        solver_free_workspace(ctx);
+        w = nullptr;
+    }
+    if (!w) {
+        w = (Workspace *)calloc(1, sizeof(Workspace));
+        if (!w) return BKR_ENOMEM;
+        ctx->ws = w;
+        w->N = N;
+        w->prec = prec;
+        w->bytes64 = field_elems(ctx->g, N) * sizeof(double2);
+        w->bytesP = field_elems(ctx->g, N) * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
+        size_t nn = (size_t)N * N * sizeof(double2);
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->C, 6 * nn));
+        w->Cprev = w->C + (size_t)N * N;
+        w->negbeta = w->C + (size_t)2 * N * N;
+        w->W = w->C + (size_t)3 * N * N;
+        w->Sinv = w->C + (size_t)4 * N * N;
+        w->Sdag = w->C + (size_t)5 * N * N;
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->bnorm2, 2 * BKR_MAX_N * sizeof(double)));
+        w->colred = w->bnorm2 + BKR_MAX_N;
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->flags, sizeof(SolverFlags)));
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->cgs, sizeof(CgScalars)));
+        BKR_CUDA(ctx, cudaMallocHost((void **)&w->h_flags, sizeof(SolverFlags)));
+        BKR_CUDA(ctx, cudaMallocHost((void **)&w->h_cgs, sizeof(CgScalars)));
+        BKR_CUDA(ctx, cudaEventCreate(&w->ev0));
+        BKR_CUDA(ctx, cudaEventCreate(&w->ev1));
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->Bn, w->bytes64));
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->Xn, w->bytes64));
+    }
+    if (block_fields && !w->Q) {
+        BKR_CUDA(ctx, cudaMalloc(&w->Q, w->bytesP));
+        BKR_CUDA(ctx, cudaMalloc(&w->Q2, w->bytesP));
+        BKR_CUDA(ctx, cudaMalloc(&w->P, w->bytesP));
+        BKR_CUDA(ctx, cudaMalloc(&w->P2, w->bytesP));
+        BKR_CUDA(ctx, cudaMalloc(&w->AP, w->bytesP));
+        if (prec != BKR_F64) {
+            BKR_CUDA(ctx, cudaMalloc((void **)&w->Y, w->bytes64));
+            BKR_CUDA(ctx, cudaMalloc((void **)&w->R64, w->bytes64));
+        } else w->R64 = (double2 *)w->AP;
+    }
+    if (cg_fields && !w->cg_r) {
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->cg_r, w->bytes64));
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->cg_p, w->bytes64));
+        BKR_CUDA(ctx, cudaMalloc((void **)&w->cg_q, w->bytes64));
+    }
+    BKR_TRY(ensure_tmp_odd(ctx, N, BKR_F64));
+    if (prec != BKR_F64) BKR_TRY(ensure_tmp_odd(ctx, N, prec));
+    return BKR_OK;
+}
+
+static int apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out, const int *done)
+{
+    BKR_TRY(launch_dslash(ctx, 1, N, prec, in, ctx->tmp_odd[prec], nullptr, 0.0, done));
+    return launch_dslash(ctx, 0, N, prec, ctx->tmp_odd[prec], out, in, 4.0 * mass * mass, done);
+}
+
+static int read_flags(bkr_ctx *ctx, Workspace *w)
+{
+    BKR_CUDA(ctx, cudaMemcpyAsync(w->h_flags, w->flags, sizeof(SolverFlags), cudaMemcpyDeviceToHost, ctx->stream));
+    BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    return BKR_OK;
+}
+
+// ----------------------------------------------------------------------------------------- blockCGrQ pieces
+
+static SmallArgs small_args(Workspace *w, int mode, int num_partials, double tol, double delta, bool mixed, bkr_ctx *ctx)
+{
+    SmallArgs a;
+    memset(&a, 0, sizeof(a));
+    a.N = w->N;
+    a.mode = mode;
+    a.num_partials = num_partials;
+    a.partials = ctx->partials;
+    a.C = w->C; a.Cprev = w->Cprev; a.negbeta = w->negbeta; a.W = w->W; a.Sinv = w->Sinv; a.Sdag = w->Sdag;
+    a.bnorm = w->bnorm2;
+    a.tol = tol; a.delta = delta;
+    a.flags = w->flags;
+    a.mixed = mixed ? 1 : 0;
+    return a;
+}
+
+// Alg. 1 l.3-l.6 (and Alg. 3 l.4-l.6 when relupd): R = B - M Xcur in fp64, thin QR, Q in inner precision, P kept.
+static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const double2 *Xcur, int small_mode, double tol,
+                             double delta, bool mixed, const int *gate)
+{
+    const int N = w->N;
+    size_t n = field_elems(ctx->g, N);
+    int np = 0;
+    BKR_TRY(apply_M(ctx, mass, N, BKR_F64, Xcur, w->R64, gate));
+    BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, w->Bn, -1.0, w->R64, w->R64, gate));
+    BKR_TRY(launch_gram_partials(ctx, N, BKR_F64, w->R64, w->R64, 1, &np, gate));
+    BKR_TRY(launch_small(ctx, small_args(w, small_mode, np, tol, delta, mixed, ctx)));
+    // Q = R C^-1 (Alg. 2 l.4), stored in the inner precision
+    return launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr);
+}
+
+// one iteration, Alg. 1 l.8-l.12
+static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, double delta, bool mixed)
+{
+    const int N = w->N, pr = w->prec;
+    const int *done = &w->flags->done;
+    int np = 0;
+    void *t;
+    // l.8  P = Q + P S^dag
+    BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done));
+    t = w->P; w->P = w->P2; w->P2 = t;
+    // l.9  beta = (P^dag M P)^-1
+    BKR_TRY(apply_M(ctx, mass, N, pr, w->P, w->AP, done));
+    BKR_TRY(launch_gram_partials(ctx, N, pr, w->P, w->AP, 1, &np, done));
+    BKR_TRY(launch_small(ctx, small_args(w, SMALL_BETA, np, tol, delta, mixed, ctx)));
+    // l.10 X = X + P (beta C)     (X in fp64 also in the mixed solver)
+    BKR_TRY(launch_block_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done));
+    // l.11 Q S = Q - (M P) beta   (thin QR = Gram + Cholesky + scale, Algorithm 2)
+    BKR_TRY(launch_block_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done));
+    BKR_TRY(launch_gram_partials(ctx, N, pr, w->Q, w->Q, 1, &np, done));
+    // l.12 C = S C, residual norms, convergence / reliable-update flags
+    BKR_TRY(launch_small(ctx, small_args(w, SMALL_QR, np, tol, delta, mixed, ctx)));
+    BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done));
+    t = w->Q; w->Q = w->Q2; w->Q2 = t;
+    return BKR_OK;
+}
+
+static int true_residuals(bkr_ctx *ctx, Workspace *w, double mass, const double2 *Xcur, double *relres_host, double *mx)
+{
+    const int N = w->N;
+    BKR_TRY(apply_M(ctx, mass, N, BKR_F64, Xcur, w->R64, nullptr));
+    BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 2, w->Bn, w->R64, w->colred, nullptr));
+    double r2[BKR_MAX_N], b2[BKR_MAX_N];
+    BKR_CUDA(ctx, cudaMemcpyAsync(r2, w->colred, N * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    BKR_CUDA(ctx, cudaMemcpyAsync(b2, w->bnorm2, N * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *mx = 0.0;
+    for (int j = 0; j < N; j++) {
+        double r = sqrt(r2[j] / b2[j]);
+        if (relres_host) relres_host[j] = r;
+        if (r > *mx) *mx = r;
+    }
+    return BKR_OK;
+}
+
+int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, double tol, int maxiter, int inner_prec,
+                 double delta, double *true_relres, bkr_stats *stats)
+{
+    const bool mixed = inner_prec == BKR_F32;
+    BKR_TRY(get_ws(ctx, N, inner_prec, true, false));
+    Workspace *w = ctx->ws;
+    w->bench_ready = false;
+    const long long launches0 = ctx->launches;
+    size_t n = field_elems(ctx->g, N);
+    BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
+    BKR_TRY(launch_pack(ctx, N, BKR_F64, X, mixed ? w->Y : w->Xn));
+    if (mixed) BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
+    BKR_CUDA(ctx, cudaEventRecord(w->ev0, ctx->stream));
+    BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 0, w->Bn, nullptr, w->bnorm2, nullptr));
+
+    int rc = BKR_OK, iters = 0, nupd = 0, restarts = 0;
+    double true_max = 0.0, iter_max = 0.0;
+    const int check_every = mixed ? 1 : 8;
+    for (;;) {
+        BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+        // l.3-l.6: R = B - M X ; Q C = R ; S = 1 ; P = 0
+        BKR_TRY(block_residual_qr(ctx, w, mass, mixed ? w->Y : w->Xn, SMALL_INIT, tol, delta, mixed, nullptr));
+        BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
+        BKR_TRY(read_flags(ctx, w));
+        int base = iters;
+        while (!w->h_flags->done && iters < maxiter) {
+            int batch = check_every < maxiter - iters ? check_every : maxiter - iters;
+            for (int b = 0; b < batch; b++) BKR_TRY(block_iteration(ctx, w, mass, tol, delta, mixed));
+            BKR_TRY(read_flags(ctx, w));
+            iters = base + w->h_flags->iters;
+            if (mixed && w->h_flags->want_update && !w->h_flags->done) {
+                // Algorithm 3: Y += X ; X = 0 ; R = B - M Y (fp64) ; Qhat C_new = R ; S = C_new Cprev^-1
+                BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, w->Y, 1.0, w->Xn, w->Y, nullptr));
+                BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
+                BKR_TRY(block_residual_qr(ctx, w, mass, w->Y, SMALL_RELUPD, tol, delta, mixed, nullptr));
+                nupd++;
+                BKR_TRY(read_flags(ctx, w));
+            }
+        }
+        iter_max = w->h_flags->relres_max;
+        if (mixed) { // result = Y + X
+            BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, w->Y, 1.0, w->Xn, w->Y, nullptr));
+            BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
+        }
+        BKR_TRY(true_residuals(ctx, w, mass, mixed ? w->Y : w->Xn, true_relres, &true_max));
+        if (w->h_flags->breakdown) { rc = BKR_EBREAKDOWN; break; }
+        if (true_max <= tol) { rc = BKR_OK; break; }
+        if (iters >= maxiter || restarts >= 8) { rc = BKR_ENOCONV; break; }
+        restarts++; // iterated residual passed but the true one missed tol (U10): re-enter from X
+    }
+    BKR_CUDA(ctx, cudaEventRecord(w->ev1, ctx->stream));
+    BKR_TRY(launch_unpack(ctx, N, BKR_F64, mixed ? w->Y : w->Xn, X));
+    BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (stats) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, w->ev0, w->ev1);
+        stats->iters = iters;
+        stats->reliable_updates = nupd;
+        stats->status = rc;
+        stats->restarts = restarts;
+        stats->seconds = ms * 1e-3;
+        stats->true_relres_max = true_max;
+        stats->iter_relres_max = iter_max;
+        stats->gpu_launches = ctx->launches - launches0;
+    }
+    return rc;
+}
+
+// ----------------------------------------------------------------------------------------- CG baseline
+
+// CG on Nc columns at once with per-column scalars (Nc = 1: the paper's sequential baseline, PAPER.md:324;
+// Nc = N: "pseudo-block").  b, x: native fp64 blocks of Nc columns.
+static int cg_loop(bkr_ctx *ctx, Workspace *w, double mass, int Nc, const double2 *b, double2 *x, double tol, int maxiter,
+                   int *iters_out, int *status)
+{
+    size_t n = field_elems(ctx->g, Nc);
+    CgScalars *s = w->cgs;
+    const int *done = &w->flags->done;
+    BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+    BKR_CUDA(ctx, cudaMemsetAsync(s, 0, sizeof(CgScalars), ctx->stream));
+    BKR_TRY(apply_M(ctx, mass, Nc, BKR_F64, x, w->cg_r, nullptr));
+    BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, b, -1.0, w->cg_r, w->cg_r, nullptr));
+    BKR_CUDA(ctx, cudaMemcpyAsync(w->cg_p, w->cg_r, n * sizeof(double2), cudaMemcpyDeviceToDevice, ctx->stream));
+    BKR_TRY(launch_col_reduce(ctx, Nc, BKR_F64, 0, w->cg_r, nullptr, s->rho, nullptr));
+    BKR_TRY(launch_col_reduce(ctx, Nc, BKR_F64, 0, b, nullptr, s->bb, nullptr));
+    BKR_TRY(launch_cg_scalar(ctx, Nc, 2, tol, s, w->flags));
+    BKR_TRY(read_flags(ctx, w));
+    int launched = 0;
+    const int check_every = 10;
+    while (!w->h_flags->done && launched < maxiter) {
+        int batch = check_every < maxiter - launched ? check_every : maxiter - launched;
+        for (int it = 0; it < batch; it++) {
+            BKR_TRY(apply_M(ctx, mass, Nc, BKR_F64, w->cg_p, w->cg_q, done));
+            BKR_TRY(launch_col_reduce(ctx, Nc, BKR_F64, 1, w->cg_p, w->cg_q, s->pAp, done));
+            BKR_TRY(launch_cg_scalar(ctx, Nc, 0, tol, s, w->flags));
+            BKR_TRY(launch_cg_update(ctx, Nc, BKR_F64, 0, s->alpha, x, w->cg_p, w->cg_r, w->cg_q, done));
+            BKR_TRY(launch_col_reduce(ctx, Nc, BKR_F64, 0, w->cg_r, nullptr, s->rho_new, done));
+            BKR_TRY(launch_cg_scalar(ctx, Nc, 1, tol, s, w->flags));
+            BKR_TRY(launch_cg_update(ctx, Nc, BKR_F64, 1, s->beta, nullptr, w->cg_p, w->cg_r, nullptr, done));
+        }
+        launched += batch;
+        BKR_TRY(read_flags(ctx, w));
+    }
+    BKR_CUDA(ctx, cudaMemcpyAsync(w->h_cgs, s, sizeof(CgScalars), cudaMemcpyDeviceToHost, ctx->stream));
+    BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int j = 0; j < Nc; j++) iters_out[j] = w->h_cgs->iters[j];
+    *status = w->h_flags->done ? BKR_OK : BKR_ENOCONV;
+    return BKR_OK;
+}
+
+int solver_cg(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, double tol, int maxiter, int batched,
+              int *iters, double *true_relres, bkr_stats *stats)
+{
+    BKR_TRY(get_ws(ctx, N, BKR_F64, false, true));
+    Workspace *w = ctx->ws;
+    w->bench_ready = false;
+    const long long launches0 = ctx->launches;
+    size_t L = (size_t)ctx->g.Vh * 3;
+    int its[BKR_MAX_N];
+    int rc = BKR_OK, st = BKR_OK, max_it = 0;
+    BKR_CUDA(ctx, cudaEventRecord(w->ev0, ctx->stream));
+    if (batched) {
+        BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
+        BKR_TRY(launch_pack(ctx, N, BKR_F64, X, w->Xn));
+        BKR_TRY(cg_loop(ctx, w, mass, N, w->Bn, w->Xn, tol, maxiter, its, &st));
+        rc = st;
+        BKR_TRY(launch_unpack(ctx, N, BKR_F64, w->Xn, X));
+    } else {
+        // a canonical column [e][a] IS the native layout for one rhs: solve in place, one rhs after the other
+        for (int j = 0; j < N; j++) {
+            BKR_TRY(cg_loop(ctx, w, mass, 1, B + (size_t)j * L, X + (size_t)j * L, tol, maxiter, its + j, &st));
+            if (st != BKR_OK) rc = st;
+        }
+    }
+    BKR_CUDA(ctx, cudaEventRecord(w->ev1, ctx->stream));
+    // true residuals of all columns (fp64), outside the timed region
+    BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
+    BKR_TRY(launch_pack(ctx, N, BKR_F64, X, w->Xn));
+    BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 0, w->Bn, nullptr, w->bnorm2, nullptr));
+    double mx = 0.0;
+    {
+        // R64 is not allocated for the CG workspace: use cg_q as the scratch block
+        double2 *save = w->R64;
+        w->R64 = w->cg_q;
+        int r2 = true_residuals(ctx, w, mass, w->Xn, true_relres, &mx);
+        w->R64 = save;
+        BKR_TRY(r2);
+    }
+    for (int j = 0; j < N; j++) {
+        if (iters) iters[j] = its[j];
+        if (its[j] > max_it) max_it = its[j];
+    }
+    if (rc == BKR_OK && mx > tol * 1.5) rc = BKR_ENOCONV;
+    if (stats) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, w->ev0, w->ev1);
+        long long tot = 0;
+        for (int j = 0; j < N; j++) tot += its[j];
+        stats->iters = batched ? max_it : (int)tot;
+        stats->reliable_updates = 0;
+        stats->status = rc;
+        stats->restarts = 0;
+        stats->seconds = ms * 1e-3;
+        stats->true_relres_max = mx;
+        stats->iter_relres_max = 0.0;
+        stats->gpu_launches = ctx->launches - launches0;
+    }
+    return rc;
+}
+
+// ----------------------------------------------------------------------------------------- bench hook
+
+int solver_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const double2 *B, int iters, long long *launches)
+{
+    BKR_TRY(get_ws(ctx, N, prec, true, false));
+    Workspace *w = ctx->ws;
+    const bool mixed = prec == BKR_F32;
+    if (!w->bench_ready) {
+        BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
+        BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
+        if (mixed) BKR_CUDA(ctx, cudaMemsetAsync(w->Y, 0, w->bytes64, ctx->stream));
+        BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 0, w->Bn, nullptr, w->bnorm2, nullptr));
+        BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+        BKR_TRY(block_residual_qr(ctx, w, mass, mixed ? w->Y : w->Xn, SMALL_INIT, 0.0, 0.0, false, nullptr));
+        BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
+        w->bench_ready = true;
+    }
+    long long l0 = ctx->launches;
+    // tol = 0: never converges, so every enqueued iteration does the full work; "mixed" flag off so that no
+    // reliable update is requested (the fp32 arithmetic of the iteration itself is what is timed).
+    for (int i = 0; i < iters; i++) BKR_TRY(block_iteration(ctx, w, mass, 0.0, 0.0, false));
+    if (launches) *launches = ctx->launches - l0;
+    return BKR_OK;
+}
