@@ -1,0 +1,444 @@
+#!/usr/bin/env python
+"""bench.py -- measurement harness.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl bkr|reference] [--workload cfg3|cfg5|cfg2]
+                    [--no-solve] [--sweep]
+
+A "step" is one blockCGrQ iteration (Algorithm 1 l.8-l.12 of arXiv:1710.09745: 2 multi-rhs Dslash, 2 Gram
+reductions, the block updates of P, X, Q and the one-CTA small-matrix kernels) on the workload's block of N rhs,
+enqueued through the C ABI (bkr_bench_iterations).  Prints ONE JSON line.
+
+  value      effective GB/s of the iteration = ALGORITHMIC bytes of one fused iteration (links twice + 14 block
+             passes) / device time per step, inputs resident in HBM;
+  e2e        the same metric through bkr_solve_block_host: host buffers in, K iterations, true-residual check,
+             host buffer out, all copies inside the timed region;
+  roofline   the dominant kernel (multi-rhs Dslash), timed alone with CUDA events on the launching stream;
+  kernels    Dslash / Gram / block-update GB/s and roofline fractions at the workload's N;
+  solve      block-CG time-to-solution and iterations against N sequential CGs and one batched CG;
+  cpu_baseline  the oracle (as it stands) on the host cores, on a bounded sample.
+
+Multi-GPU: the path does not shard: "replicas only" -- every rank runs the same step on its
+own GPU with no data-path collective, value = sum over ranks / max time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOADS = {
+    # name: (BASELINE.json config, dims, link kind, mass, N)
+    "cfg2": ("configs[1]: 16^4, N=8, m=0.05", (16, 16, 16, 16), "perturbed", 0.05, 8),
+    "cfg3": ("configs[2]: 32^3x64, N=16, m=0.01", (32, 32, 32, 64), "perturbed", 0.01, 16),
+    "cfg5": ("configs[4]: 32^4 kernel sweep, N=16", (32, 32, 32, 32), "random", 0.05, 16),
+}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ---------------------------------------------------------------- algorithmic bytes / flops
+
+def volume(dims):
+    v = 1
+    for d in dims:
+        v *= d
+    return v
+
+
+def bytes_dslash(dims, N, w, xpay=False):
+    return w * volume(dims) * (144 + 6 * N + (3 * N if xpay else 0))
+
+
+def flops_dslash(dims, N, xpay=False):
+    return (1158 if xpay else 1146) * (volume(dims) // 2) * N
+
+
+def block_bytes(dims, N, w):
+    return 2 * w * 3 * (volume(dims) // 2) * N
+
+
+def bytes_iteration(dims, N, w):
+    """fused-iteration traffic: links twice + 14 block passes."""
+    return 2 * 144 * w * volume(dims) + 14 * block_bytes(dims, N, w)
+
+
+def flops_iteration(dims, N):
+    L = 3 * (volume(dims) // 2)
+    return 2304 * (volume(dims) // 2) * N + 36 * L * N * N
+
+
+# ---------------------------------------------------------------- clocks sampler
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ---------------------------------------------------------------- timing helpers
+
+def time_loop(torch, fn, reps, warmup):
+    """average ms per call of fn over `reps` calls, CUDA events on the current (= the library's) stream."""
+    for _ in range(warmup):
+        fn()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
+    """Dslash / Gram / block-update timings at one (N, precision): dict of GB/s, GFLOPS, fraction of HBM peak."""
+    w = 8 if prec == binding.F64 else 4
+    L = ctx.L
+    nb = 3  # rotate over several buffers so that small blocks are not served from L2 alone
+    blk = [ctx.empty_native(N, prec).normal_() for _ in range(nb + 1)]
+    a = torch.randn(N, N, dtype=torch.complex128, device=ctx.device) * 0.1
+    K = torch.empty(N, N, dtype=torch.complex128, device=ctx.device)
+    out = {}
+    i = [0]
+
+    def rot():
+        i[0] = (i[0] + 1) % nb
+        return blk[i[0]], blk[(i[0] + 1) % nb]
+
+    def f_dslash():
+        s, d = rot()
+        ctx.dslash(i[0] & 1, N, s, d, prec)
+    ms = time_loop(torch, f_dslash, reps, warmup)
+    by, fl = bytes_dslash(dims, N, w), flops_dslash(dims, N)
+    out["dslash"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+
+    def f_gram2():
+        s, d = rot()
+        ctx.gram(N, s, d, hermitian=False, prec=prec, out=K)
+    ms = time_loop(torch, f_gram2, reps, warmup)
+    by, fl = 2 * block_bytes(dims, N, w), 8 * L * N * N
+    out["gram_xy"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+
+    def f_gram1():
+        s, _ = rot()
+        ctx.gram(N, s, s, hermitian=True, prec=prec, out=K)
+    ms = time_loop(torch, f_gram1, reps, warmup)
+    by, fl = block_bytes(dims, N, w), 4 * L * N * (N + 1)
+    out["gram_xx"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+
+    def f_axpy():
+        s, d = rot()
+        ctx.block_axpy(N, a, s, d, prec)
+    ms = time_loop(torch, f_axpy, reps, warmup)
+    by, fl = 3 * block_bytes(dims, N, w), 8 * L * N * N
+    out["block_axpy"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+    return out
+
+
+# ---------------------------------------------------------------- CPU baseline (the oracle, as it stands)
+
+def oracle_sample(dims_full, N, kind, seed=5):
+    """One blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update) with the oracle on a bounded
+    sample: the same N and link generator on a lattice shrunk until it is ~10-30 s of CPU work.
+    returns (seconds, algorithmic bytes of the sample, sample description, threads)."""
+    import numpy as np
+    import oracle
+    from paper_1710_09745_b200 import synth
+    dims = list(dims_full)
+    while volume(dims) * N > 32 ** 4 * 16:  # ~4 s on 8 cores = about 30 s of CPU work
+        k = max(range(4), key=lambda mu: dims[mu])
+        dims[k] //= 2
+    dims = tuple(dims)
+    fat, lng = synth.make_links(dims, kind, seed)
+    fat, lng = fat.numpy(), lng.numpy()
+    P = synth.make_sources(dims, N, seed + 1).numpy()
+    Q = synth.make_sources(dims, N, seed + 2).numpy()
+    a = (np.eye(N) * 0.5).astype(np.complex128)
+    oracle.lib()
+    t0 = time.perf_counter()
+    AP = oracle.apply_M(dims, fat, lng, 0.05, P)
+    oracle.gram(P, AP)
+    oracle.gram(Q, Q)
+    for _ in range(4):
+        oracle.block_axpy(a, P, Q)
+    dt = time.perf_counter() - t0
+    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    desc = "one blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update), N=%d, on a %s lattice" % (
+        N, "x".join(str(d) for d in dims))
+    return dt, bytes_iteration(dims, N, 8), desc, threads
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/unit/config, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    name, dims, kind, mass, N = WORKLOADS[args.workload]
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt, by, desc, threads = oracle_sample(dims, N, kind)
+        if i >= args.warmup:
+            times.append(dt)
+        if sum(times) > 150:
+            break
+    ms = 1e3 * sum(times) / len(times)
+    val = by / ms * 1e-6
+    line = {
+        "impl": "reference", "metric": "blockcg_iteration_effective_GBps", "value": val, "unit": "GB/s",
+        "n_gpus": args.gpus, "steps": len(times), "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": name, "dims": list(dims), "N": N, "mass": mass, "links": kind},
+        "cpu_baseline": {"value": val, "unit": "GB/s", "cores": threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": "GB/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ---------------------------------------------------------------- the CUDA path
+
+def run_bkr(args):
+    import torch
+    from paper_1710_09745_b200 import binding, synth
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm, peak_src = peaks()
+    name, dims, kind, mass, N = WORKLOADS[args.workload]
+    if args.N:
+        N = args.N
+    prec = binding.F32 if args.prec == "f32" else binding.F64
+    w = 8 if prec == binding.F64 else 4
+    dev = "cuda:%d" % local
+
+    # inputs: seeded synthetic links and sources drawn on the device (synth.py), resident in HBM
+    fat, lng = synth.make_links(dims, kind, seed=1000 + rank, device=dev)
+    B = synth.make_sources(dims, N, seed=2000 + rank, device=dev)
+    ctx = binding.Context(dims, device=local)
+    ctx.load_links(fat, lng, also_f32=True)
+    del fat, lng
+    torch.cuda.empty_cache()
+
+    # ---- timed region: K iterations after W warm-up iterations, device-resident
+    launches_w = ctx.bench_iterations(mass, B, args.warmup, prec)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    launches = ctx.bench_iterations(mass, B, args.steps, prec)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    ms_total = e0.elapsed_time(e1)
+    if dist:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    by_iter = bytes_iteration(dims, N, w)
+    value = world * by_iter / ms_step * 1e-6
+
+    # ---- the dominant kernel alone (multi-rhs Dslash), and the multi-BLAS kernels, at this N
+    kern = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=max(10, args.steps), warmup=3, hbm=hbm)
+    clocks = sampler.stop()
+
+    # ---- end to end through the host-buffer entry point (copies inside the timed region)
+    e2e = None
+    if rank == 0 or dist:
+        Bh = B.cpu().pin_memory()
+        Xh = torch.zeros_like(Bh).pin_memory()
+        ctx.solve_block_host(mass, Bh, Xh, tol=1e-10, maxiter=2, inner_prec=prec)  # warm-up (allocations)
+        Xh.zero_()
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        t0 = time.perf_counter()
+        rr, st = ctx.solve_block_host(mass, Bh, Xh, tol=1e-10, maxiter=args.steps, inner_prec=prec)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if dist:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        k = max(1, st["iters"])
+        e2e = {"value": world * k * by_iter / dt * 1e-9, "unit": "GB/s",
+               "h2d_bytes_per_step": 2 * Bh.numel() * 16 / k, "d2h_bytes_per_step": Xh.numel() * 16 / k,
+               "iterations": k, "seconds": dt,
+               "note": "bkr_solve_block_host: H2D of B and X0, init QR, %d iterations, fp64 true-residual check, D2H of X" % k}
+        del Bh, Xh
+
+    # ---- time to solution: block CG vs N x CG (rank 0, N = 1 GPU runs only)
+    solve = None
+    if rank == 0 and world == 1 and not args.no_solve:
+        solve = solve_comparison(torch, ctx, binding, mass, B, args)
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return 0
+
+    cpu = None
+    if world == 1 and not args.no_cpu:
+        dt, sby, desc, threads = oracle_sample(dims, N, kind)
+        cpu = {"value": sby / dt * 1e-9, "unit": "GB/s", "cores": threads, "kind": "oracle", "sample": desc,
+               "seconds": dt}
+
+    d = kern["dslash"]
+    line = {
+        "metric": "blockcg_iteration_effective_GBps", "value": value, "unit": "GB/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == binding.F64 else "f32", "data": "synthetic",
+        "config": {"workload": name, "dims": list(dims), "N": N, "mass": mass, "links": kind,
+                   "step": "one blockCGrQ iteration (Alg. 1 l.8-12): 2 Dslash, 2 Gram, P/X/Q block updates, small-matrix kernels",
+                   "l2": "inputs larger than L2 (links %.2f GB + blocks %.2f GB each)" % (
+                       144 * w * volume(dims) * 1e-9, block_bytes(dims, N, w) * 1e-9),
+                   "parallelism": "replicas only" if world > 1 else "1 GPU"},
+        "frac_hbm_iteration": value / world / hbm,
+        "GFLOPS_iteration": world * flops_iteration(dims, N) / ms_step * 1e-6,
+        "roofline": {"bound": "hbm", "kernel": "dslash_kernel (multi-rhs Dslash, one parity, N=%d)" % N,
+                     "achieved": d["GBps"], "peak": hbm, "unit": "GB/s", "frac": d["GBps"] / hbm, "traffic": None,
+                     "peak_source": peak_src, "ms_per_launch": d["ms"],
+                     "algorithmic_bytes_per_launch": bytes_dslash(dims, N, w), "GFLOPS": d["GFLOPS"]},
+        "kernels": kern,
+        "e2e": e2e,
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "cpu_baseline": cpu,
+        "solve": solve,
+    }
+    print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def solve_comparison(torch, ctx, binding, mass, B, args):
+    """block CG vs N sequential CGs vs one batched CG, tol 1e-10 (north_star).  Sequential CG is measured on
+    `--cg-rhs` right-hand sides and scaled to N (stated in the output)."""
+    N = int(B.shape[0])
+    out = {"tol": 1e-10, "N": N}
+    X, rr, st = ctx.solve_block(mass, B, tol=1e-10, maxiter=args.maxiter)
+    out["block_cg"] = {"seconds": st["seconds"], "iters": st["iters"], "status": st["status"], "restarts": st["restarts"],
+                       "true_relres_max": max(rr)}
+    X, rr, st = ctx.solve_block(mass, B, tol=1e-10, maxiter=args.maxiter, inner_prec=binding.F32, delta=0.1)
+    out["block_cg_mixed"] = {"seconds": st["seconds"], "iters": st["iters"], "status": st["status"],
+                             "reliable_updates": st["reliable_updates"], "true_relres_max": max(rr)}
+    n_seq = min(N, args.cg_rhs)
+    X, its, rr, st = ctx.solve_cg(mass, B[:n_seq].contiguous(), tol=1e-10, maxiter=args.maxiter, batched=False)
+    out["cg_sequential"] = {"seconds": st["seconds"] * N / n_seq, "measured_rhs": n_seq, "scaled_to": N,
+                            "iters_mean": sum(its) / len(its), "status": st["status"], "true_relres_max": max(rr)}
+    X, its, rr, st = ctx.solve_cg(mass, B, tol=1e-10, maxiter=args.maxiter, batched=True)
+    out["cg_batched"] = {"seconds": st["seconds"], "iters_max": max(its), "status": st["status"], "true_relres_max": max(rr)}
+    out["speedup_vs_sequential_cg"] = out["cg_sequential"]["seconds"] / out["block_cg"]["seconds"]
+    out["speedup_vs_batched_cg"] = out["cg_batched"]["seconds"] / out["block_cg"]["seconds"]
+    out["paper_context"] = "paper: 5x over sequential CG on SaturnV (PAPER.md:27, 370-378), other hardware and real ensembles"
+    return out
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: 32^4, random SU(3), N in {1,2,4,8,16,24,32}, fp64 and fp32: one JSON line per point."""
+    import torch
+    from paper_1710_09745_b200 import binding, synth
+    hbm, _ = peaks()
+    name, dims, kind, mass, _ = WORKLOADS["cfg5"]
+    fat, lng = synth.make_links(dims, kind, seed=1000, device="cuda")
+    ctx = binding.Context(dims)
+    ctx.load_links(fat, lng, also_f32=True)
+    del fat, lng
+    for prec, pname in ((binding.F64, "f64"), (binding.F32, "f32")):
+        for N in (1, 2, 4, 8, 16, 24, 32):
+            k = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=args.steps, warmup=3, hbm=hbm)
+            row = {"sweep": name, "dtype": pname, "N": N}
+            for kn, v in k.items():
+                row[kn] = {a: round(b, 4) for a, b in v.items()}
+            print(json.dumps(row), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="bkr", choices=["bkr", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--N", type=int, default=0)
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--no-solve", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--maxiter", type=int, default=20000)
+    ap.add_argument("--cg-rhs", type=int, default=2, help="sequential CG is measured on this many rhs and scaled to N")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "bkr" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
+    return run_bkr(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -111,11 +111,15 @@ class Context:
             raise BkrError(rc, "bkr_create")
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().bkr_destroy(self._h)
-            self._h = None
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.bkr_destroy(self._h)
+        self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:  # interpreter shutdown: the library may already be gone
+            pass
 
     def _check(self, rc, where, allow=()):
         if rc != OK and rc not in allow:

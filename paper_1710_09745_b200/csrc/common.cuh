@@ -121,7 +121,7 @@ struct SmallArgs {
     double2 *negbeta, *W;    // -beta and W = beta C  (Alg. 1 l.9, l.10)
     double2 *Sinv, *Sdag;    // S^-1 and S^dagger (Alg. 1 l.11 / l.8)
     double2 *out0, *out1;    // API path outputs
-    const double *bnorm;     // ||b_i||
+    const double *bnorm2;    // ||b_i||^2
     double tol, delta;
     SolverFlags *flags;
     int *status;             // API path

@@ -25,11 +25,17 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 b) // conj(a) * b
 
 // In-place upper Cholesky of the Hermitian matrix whose upper triangle is in A (row-major, shared memory).
 // On return A = R (upper triangular, real positive diagonal, zeros below).  One warp; lane = column.
+//
+// Breakdown (U15): a pivot that is non-finite, non-positive, or has lost more than 13
+// digits against the diagonal entry it started from (d <= 1e-13 h_jj: the column is linearly dependent on the
+// previous ones to working precision, and only rounding noise decides the sign of the pivot).
 __device__ bool warp_cholesky_upper(int N, double2 *A, int lane)
 {
+    const double h0 = lane < N ? A[lane * N + lane].x : 0.0;
     for (int j = 0; j < N; j++) {
         double d = A[j * N + j].x;
-        if (!(d > 0.0) || !isfinite(d)) return false; // uniform across the warp
+        double hjj = __shfl_sync(0xffffffffu, h0, j);
+        if (!(d > 1e-13 * hjj) || !isfinite(d)) return false; // uniform across the warp
         double rjj = sqrt(d);
         __syncwarp();
         if (lane < N) {
@@ -96,7 +102,7 @@ __device__ void load_hermitian(const SmallArgs &p, double2 *A)
 }
 
 // residual norms from C (PAPER.md:208 with the index fix U11): r_i = ||C[:,i]|| / ||b_i||
-__device__ double max_relres(int N, const double2 *C, const double *bnorm, double *scratch)
+__device__ double max_relres(int N, const double2 *C, const double *bnorm2, double *scratch)
 {
     for (int i = threadIdx.x; i < N; i += blockDim.x) {
         double s = 0.0;
@@ -104,7 +110,7 @@ __device__ double max_relres(int N, const double2 *C, const double *bnorm, doubl
             double2 v = C[j * N + i];
             s += v.x * v.x + v.y * v.y;
         }
-        scratch[i] = sqrt(s) / bnorm[i];
+        scratch[i] = sqrt(s / bnorm2[i]);
     }
     __syncthreads();
     double m = 0.0;
@@ -209,7 +215,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
             p.C[o] = s;
         }
         __syncthreads();
-        double r = max_relres(N, Cm, p.bnorm, scratch);
+        double r = max_relres(N, Cm, p.bnorm2, scratch);
         if (threadIdx.x == 0) {
             fl->iters += 1;
             fl->relres_max = r;
@@ -227,7 +233,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
             p.Sinv[o] = B[o];
             p.Sdag[o] = make_double2(i == j ? 1.0 : 0.0, 0.0);
         }
-        double r = max_relres(N, A, p.bnorm, scratch);
+        double r = max_relres(N, A, p.bnorm2, scratch);
         if (threadIdx.x == 0) {
             fl->relres_max = r;
             fl->relres_last_update = r;
@@ -260,7 +266,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
             p.Sinv[o] = B[o];
             p.C[o] = A[o];
         }
-        double r = max_relres(N, A, p.bnorm, scratch);
+        double r = max_relres(N, A, p.bnorm2, scratch);
         if (threadIdx.x == 0) {
             fl->relres_max = r;
             fl->relres_last_update = r;

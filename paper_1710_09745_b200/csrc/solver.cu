@@ -136,7 +136,7 @@ static SmallArgs small_args(Workspace *w, int mode, int num_partials, double tol
     a.num_partials = num_partials;
     a.partials = ctx->partials;
     a.C = w->C; a.Cprev = w->Cprev; a.negbeta = w->negbeta; a.W = w->W; a.Sinv = w->Sinv; a.Sdag = w->Sdag;
-    a.bnorm = w->bnorm2;
+    a.bnorm2 = w->bnorm2;
     a.tol = tol; a.delta = delta;
     a.flags = w->flags;
     a.mixed = mixed ? 1 : 0;
