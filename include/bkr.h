@@ -27,9 +27,11 @@
  *                                        multiplied in; backward hops use U(x - h mu)^dagger (eq. 2).
  *  canonical vector  v[rhs][e][a]        e = s div 2 = even-odd index of a site of the field's parity,
  *                                        a = colour 0..2; a parity field has Vh = XYZT/2 sites.
- *  native block      v[e][a][rhs]        the L x N "composite field" of PAPER.md:176, 212-216 stored
- *                                        row-major (row k = 3 e + a, L = 3 Vh; the N rhs of one row are
- *                                        contiguous).  bkr_field_bytes() bytes, 256-byte aligned base.
+ *  native block      v[rhs][a][e]        the L x N "composite field" of PAPER.md:176, 212-216: N vectors of
+ *                                        L = 3 Vh complex stored one after the other (component j is the
+ *                                        contiguous view at offset j*L); inside a vector, row k = a*Vh + e
+ *                                        (colour planes, SoA over sites).  bkr_field_bytes() bytes, 16-byte
+ *                                        aligned base.
  *  small matrices    a[i][j]             N x N complex fp64, row-major, device memory.
  */
 #ifndef BKR_H
@@ -82,7 +84,7 @@ int bkr_load_links(bkr_ctx *ctx, const void *fat, const void *lng, int also_f32)
 /* Bytes of one native block of N rhs on one parity in precision prec (0 on bad arguments). */
 size_t bkr_field_bytes(const bkr_ctx *ctx, int N, int prec);
 
-/* canonical fp64 [rhs][e][a]  <->  native [e][a][rhs] in precision prec. */
+/* canonical fp64 [rhs][e][a]  <->  native [rhs][a][e] in precision prec. */
 int bkr_pack(bkr_ctx *ctx, int N, int prec, const void *canonical, void *native);
 int bkr_unpack(bkr_ctx *ctx, int N, int prec, const void *native, void *canonical);
 

@@ -138,7 +138,7 @@ class Context:
         return int(lib().bkr_field_bytes(self._h, int(N), int(prec)))
 
     def empty_native(self, N, prec=F64):
-        """uninitialised native block [e][a][rhs] as a flat real tensor (fp64 or fp32)."""
+        """uninitialised native block [rhs][a][e] as a flat real tensor (fp64 or fp32)."""
         dt = torch.float64 if prec == F64 else torch.float32
         return torch.empty(self.L * int(N) * 2, dtype=dt, device=self.device)
 

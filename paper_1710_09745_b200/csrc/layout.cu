@@ -1,9 +1,11 @@
 // Field and link layouts ("reordering the vector and link fields to achieve memory
 // coalescing"; PAPER.md:212-216 composite fields).  See DESIGN.md section 5.
 //
-//   native block  v[e][a][j]     : L x N row-major, the N rhs of a (site, colour) row contiguous, so that a
-//                                  neighbour gather in the stencil is one contiguous 6*N*w-byte read and the
-//                                  block BLAS sees plain row-major tall-skinny matrices.
+//   native block  v[j][a][e]     : N vectors of L = 3 Vh complex each, stored one after the other ("composite
+//                                  field" whose components are contiguous views); inside a
+//                                  vector the three colour planes are SoA over the even-odd site index, so a
+//                                  warp of 32 consecutive sites (stencil) or rows (block BLAS) reads 512
+//                                  contiguous bytes per instruction in fp64.
 //   native links  L[d][el][e]    : d = (type*4 + mu)*2 + parity, el = 3*row + col; complex SoA over sites, so
 //                                  the lanes of a warp that work on different sites read contiguous 16 B
 //                                  (fp64) / 8 B (fp32) pieces and lanes on the same site broadcast.
@@ -45,70 +47,53 @@ int launch_pack_links(bkr_ctx *ctx, const double2 *fat, const double2 *lng, doub
     return bkr_check_launch(ctx);
 }
 
-// canonical [j][e][a] fp64  <->  native [e][a][j].  A 32 x 32 shared-memory transpose over (row k, rhs j)
-// keeps both sides coalesced.
+// canonical [j][e][a] fp64  <->  native [j][a][e]: a 3 x Vh transpose per rhs.  One thread per (e, j); the
+// native side is coalesced (32 consecutive sites of one plane per warp instruction), the canonical side reads or
+// writes 48 contiguous bytes per thread.  Not on the hot path (boundary of the solve calls only).
 template <typename Real, bool PACK>
-__global__ void transpose_kernel(size_t L, int N, const double2 *__restrict__ canon_in, double2 *__restrict__ canon_out,
+__global__ void transpose_kernel(size_t Vh, int N, const double2 *__restrict__ canon_in, double2 *__restrict__ canon_out,
                                  const typename CxT<Real>::type *__restrict__ nat_in,
                                  typename CxT<Real>::type *__restrict__ nat_out)
 {
     typedef typename CxT<Real>::type Cx;
-    __shared__ double2 tile[32][33];
-    size_t k0 = (size_t)blockIdx.x * 32;
-    int tx = threadIdx.x, ty = threadIdx.y; // 32 x 8
-    if (PACK) {
-        for (int j = ty; j < N; j += 8) {
-            size_t k = k0 + tx;
-            if (k < L) tile[j][tx] = canon_in[(size_t)j * L + k];
-        }
-        __syncthreads();
-        for (int kk = ty; kk < 32; kk += 8) {
-            size_t k = k0 + kk;
-            if (k < L && tx < N) {
-                double2 v = tile[tx][kk];
-                Cx o;
-                o.x = (Real)v.x;
-                o.y = (Real)v.y;
-                nat_out[k * N + tx] = o;
-            }
-        }
-    } else {
-        for (int kk = ty; kk < 32; kk += 8) {
-            size_t k = k0 + kk;
-            if (k < L && tx < N) {
-                Cx v = nat_in[k * N + tx];
-                tile[tx][kk] = make_double2((double)v.x, (double)v.y);
-            }
-        }
-        __syncthreads();
-        for (int j = ty; j < N; j += 8) {
-            size_t k = k0 + tx;
-            if (k < L) canon_out[(size_t)j * L + k] = tile[j][tx];
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (e >= Vh) return;
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+        const size_t ic = ((size_t)j * Vh + e) * 3 + a, in = ((size_t)j * 3 + a) * Vh + e;
+        if (PACK) {
+            const double2 v = canon_in[ic];
+            Cx o;
+            o.x = (Real)v.x;
+            o.y = (Real)v.y;
+            nat_out[in] = o;
+        } else {
+            const Cx v = nat_in[in];
+            canon_out[ic] = make_double2((double)v.x, (double)v.y);
         }
     }
 }
 
 int launch_pack(bkr_ctx *ctx, int N, int prec, const double2 *canonical, void *native)
 {
-    size_t L = (size_t)ctx->g.Vh * 3;
-    dim3 block(32, 8);
-    unsigned blocks = (unsigned)((L + 31) / 32);
+    size_t Vh = (size_t)ctx->g.Vh;
+    dim3 grid((unsigned)((Vh + 255) / 256), N);
     if (prec == BKR_F64)
-        transpose_kernel<double, true><<<blocks, block, 0, ctx->stream>>>(L, N, canonical, nullptr, nullptr, (double2 *)native);
+        transpose_kernel<double, true><<<grid, 256, 0, ctx->stream>>>(Vh, N, canonical, nullptr, nullptr, (double2 *)native);
     else
-        transpose_kernel<float, true><<<blocks, block, 0, ctx->stream>>>(L, N, canonical, nullptr, nullptr, (float2 *)native);
+        transpose_kernel<float, true><<<grid, 256, 0, ctx->stream>>>(Vh, N, canonical, nullptr, nullptr, (float2 *)native);
     return bkr_check_launch(ctx);
 }
 
 int launch_unpack(bkr_ctx *ctx, int N, int prec, const void *native, double2 *canonical)
 {
-    size_t L = (size_t)ctx->g.Vh * 3;
-    dim3 block(32, 8);
-    unsigned blocks = (unsigned)((L + 31) / 32);
+    size_t Vh = (size_t)ctx->g.Vh;
+    dim3 grid((unsigned)((Vh + 255) / 256), N);
     if (prec == BKR_F64)
-        transpose_kernel<double, false><<<blocks, block, 0, ctx->stream>>>(L, N, nullptr, canonical, (const double2 *)native, nullptr);
+        transpose_kernel<double, false><<<grid, 256, 0, ctx->stream>>>(Vh, N, nullptr, canonical, (const double2 *)native, nullptr);
     else
-        transpose_kernel<float, false><<<blocks, block, 0, ctx->stream>>>(L, N, nullptr, canonical, (const float2 *)native, nullptr);
+        transpose_kernel<float, false><<<grid, 256, 0, ctx->stream>>>(Vh, N, nullptr, canonical, (const float2 *)native, nullptr);
     return bkr_check_launch(ctx);
 }
 

@@ -323,23 +323,21 @@ int solver_cg(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, do
     int its[BKR_MAX_N];
     int rc = BKR_OK, st = BKR_OK, max_it = 0;
     BKR_CUDA(ctx, cudaEventRecord(w->ev0, ctx->stream));
+    BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
+    BKR_TRY(launch_pack(ctx, N, BKR_F64, X, w->Xn));
     if (batched) {
-        BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
-        BKR_TRY(launch_pack(ctx, N, BKR_F64, X, w->Xn));
         BKR_TRY(cg_loop(ctx, w, mass, N, w->Bn, w->Xn, tol, maxiter, its, &st));
         rc = st;
-        BKR_TRY(launch_unpack(ctx, N, BKR_F64, w->Xn, X));
     } else {
-        // a canonical column [e][a] IS the native layout for one rhs: solve in place, one rhs after the other
+        // component j of a native block is the contiguous vector at offset j L: one rhs after the other
         for (int j = 0; j < N; j++) {
-            BKR_TRY(cg_loop(ctx, w, mass, 1, B + (size_t)j * L, X + (size_t)j * L, tol, maxiter, its + j, &st));
+            BKR_TRY(cg_loop(ctx, w, mass, 1, w->Bn + (size_t)j * L, w->Xn + (size_t)j * L, tol, maxiter, its + j, &st));
             if (st != BKR_OK) rc = st;
         }
     }
+    BKR_TRY(launch_unpack(ctx, N, BKR_F64, w->Xn, X));
     BKR_CUDA(ctx, cudaEventRecord(w->ev1, ctx->stream));
     // true residuals of all columns (fp64), outside the timed region
-    BKR_TRY(launch_pack(ctx, N, BKR_F64, B, w->Bn));
-    BKR_TRY(launch_pack(ctx, N, BKR_F64, X, w->Xn));
     BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 0, w->Bn, nullptr, w->bnorm2, nullptr));
     double mx = 0.0;
     {

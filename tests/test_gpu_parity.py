@@ -57,12 +57,12 @@ def test_pack_unpack_roundtrip_bit_exact(lat_asym, N):
     dims, _, _, ctx = lat_asym
     v = torch.from_numpy(H.np_sources(dims, N, 5)).cuda()
     nat = ctx.pack(v)
-    # native layout is [e][a][rhs] (include/bkr.h): check it directly, then the round trip
-    want = v.permute(1, 2, 0).contiguous()
-    assert torch.equal(torch.view_as_complex(nat.view(-1, 2)).view(ctx.Vh, 3, N), want)
+    # native layout is [rhs][a][e] (include/bkr.h): check it directly, then the round trip
+    want = v.permute(0, 2, 1).contiguous()
+    assert torch.equal(torch.view_as_complex(nat.view(-1, 2)).view(N, 3, ctx.Vh), want)
     assert torch.equal(ctx.unpack(nat, N), v)
     nat32 = ctx.pack(v, binding.F32)
-    assert torch.equal(torch.view_as_complex(nat32.view(-1, 2)).view(ctx.Vh, 3, N), want.to(torch.complex64))
+    assert torch.equal(torch.view_as_complex(nat32.view(-1, 2)).view(N, 3, ctx.Vh), want.to(torch.complex64))
 
 
 # ------------------------------------------------------------------ operator
