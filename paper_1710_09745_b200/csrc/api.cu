@@ -46,6 +46,7 @@ int bkr_destroy(bkr_ctx *ctx)
     solver_free_workspace(ctx);
     cudaFree(ctx->links64);
     cudaFree(ctx->links32);
+    cudaFree(ctx->tile_order);
     cudaFree(ctx->tmp_odd[0]);
     cudaFree(ctx->tmp_odd[1]);
     cudaFree(ctx->partials);
@@ -57,7 +58,7 @@ int bkr_destroy(bkr_ctx *ctx)
 int bkr_load_links(bkr_ctx *ctx, const void *fat, const void *lng, int also_f32)
 {
     if (!ctx || !fat || !lng) return BKR_EINVAL;
-    size_t n = (size_t)2 * 4 * ctx->g.V * 9;
+    size_t n = link_elems(ctx->g);
     if (!ctx->links64) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->links64, n * sizeof(double2)));
     if (also_f32 && !ctx->links32) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->links32, n * sizeof(float2)));
     return launch_pack_links(ctx, (const double2 *)fat, (const double2 *)lng, ctx->links64,

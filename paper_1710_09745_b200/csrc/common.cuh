@@ -7,6 +7,7 @@
 #include "../../include/bkr.h"
 
 #define BKR_NUM_SMS 148 /* B200: 2 dies x 74 SMs; grids are sized in multiples of this */
+#define BKR_LINK_TILE 64 /* sites per link tile: one TMA bulk copy per (tile, hop) = 9 * 64 complex */
 
 struct Geom {
     int X[4];     // extents x,y,z,t (all even, >= 4)
@@ -34,9 +35,12 @@ struct bkr_ctx {
     cudaStream_t stream;
     int last_cuda;
     long long launches;
-    // links in the device layout L[((type*4+mu)*2+parity)*9+el][e], type 0 fat / 1 long
+    // gather-form links Wt[parity][tile][hop][el][lane] (layout.cu), fp64 and optional fp32 copy
     double2 *links64;
     float2 *links32;
+    // tile processing order of the stencil (L2 blocking, dslash.cu): device table + the blocking it was built for
+    int *tile_order;
+    int tile_order_key;
     // scratch for apply_M (odd-parity temporary), grown on demand, per precision
     void *tmp_odd[2];
     size_t tmp_odd_bytes[2];
@@ -76,6 +80,8 @@ static inline int bkr_check_launch(bkr_ctx *ctx)
 }
 
 static inline size_t field_elems(const Geom &g, int N) { return (size_t)g.Vh * 3 * (size_t)N; }
+static inline int link_tiles(const Geom &g) { return (g.Vh + BKR_LINK_TILE - 1) / BKR_LINK_TILE; }
+static inline size_t link_elems(const Geom &g) { return (size_t)2 * link_tiles(g) * 16 * 9 * BKR_LINK_TILE; }
 
 // ---- layout.cu
 int launch_pack_links(bkr_ctx *ctx, const double2 *fat, const double2 *lng, double2 *out64, float2 *out32);

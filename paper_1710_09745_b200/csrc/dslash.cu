@@ -1,63 +1,228 @@
 // Multi-rhs improved-staggered stencil ("Dslash"), PAPER.md:95-101 (eq. 2) and PAPER.md:218-232.
 //
-//   out(x) = sum_mu [ F_mu(x) in(x+mu) - F_mu(x-mu)^dag in(x-mu) + K_mu(x) in(x+3mu) - K_mu(x-3mu)^dag in(x-3mu) ]
+//   out(x) = sum_h W_h(x) in(nbr_h(x)),  16 hops h = (mu, fat|long, forward|backward)  (gather-form links, layout.cu)
 //   optional epilogue  out = a * xp - out   (second half of M = 4 m^2 - D_eo D_oe)
 //
-// Mapping.  One thread = one output site x T right-hand sides (register tile, the
-// paper's "register tiling" PAPER.md:232); threadIdx.y = rhs group g (rhs g*T .. g*T+T-1), so the G = ceil(N/T)
-// warps that work on the same 32 sites sit in one CTA and the second..G-th read of a link hits L1 (the paper's
-// "cache tiling").  With the SoA layouts v[j][a][e] and L[d][el][e] every load instruction of a
-// warp reads 32 consecutive sites of one plane: 512 contiguous bytes in fp64.  Each link matrix is held in
-// registers (18 reals) and reused for the T vectors; links are read with evict-first hints (used once per call),
-// results are written with streaming stores, neighbour vectors use the default policy so that the x/y reuse is
-// served by L1 and the z/t reuse by L2.
-//
-// Per site and rhs: 16 x 36 = 576 FMAs (1152 flop; the paper counts 1146).  At N = 16 in fp64 the
-// three per-SM budgets are within 25 % of each other (HBM 166 clk/site, FP64 pipe 144, L1->register 132), see
-// DESIGN.md section 7.
+// Design.
+//  * One thread = one output site x T right-hand sides (the paper's register tiling); threadIdx.y =
+//    rhs group, so the G = ceil(N/T) groups that work on the same 64 sites share one CTA and one copy of the links
+//    (the paper's cache tiling, with shared memory in place of L1).
+//  * Links are a pure HBM stream: every matrix is used once per call and, at N <= 16, they are more than half of
+//    all bytes.  They never touch registers or the LSU miss path until they are needed: a persistent CTA walks
+//    over its tiles and an elected thread streams the (tile, hop) chunks -- 9 x 64 complex, contiguous in the
+//    tile-major layout -- into a 4-deep shared-memory ring with 1-D TMA bulk copies (cp.async.bulk + mbarrier
+//    complete_tx), three hops ahead of the arithmetic.  Measured on the previous LDG-only kernel: 7.9 warps of 12
+//    stalled on the long scoreboard with the FP64 pipe 33 % busy, whatever the register tile.
+//  * Neighbour vectors are read with plain 16-byte loads: a warp reads 32 consecutive sites of one (rhs, colour)
+//    plane, 512 contiguous bytes in fp64; x/y reuse comes from L1, z/t reuse from L2.
+//  * L2 blocking: tiles are visited in an order that sweeps t inside a (y, z) block, so that the 7 time slices a
+//    block needs for its t +- 1, +- 3 hops stay L2-resident (tile_order, built on the host below).
+//  * Per site and rhs: 16 x 36 = 576 FMAs (1152 flop; the paper counts 1146).
 #include "common.cuh"
 
-template <typename Real> struct LdSt;
-template <> struct LdSt<double> {
-    static __device__ __forceinline__ double2 link(const double2 *p) { return __ldcs(p); }
-    static __device__ __forceinline__ double2 vec(const double2 *p) { return __ldg(p); }
-    static __device__ __forceinline__ void out(double2 *p, double2 v) { __stcs(p, v); }
-};
-template <> struct LdSt<float> {
-    static __device__ __forceinline__ float2 link(const float2 *p) { return __ldcs(p); }
-    static __device__ __forceinline__ float2 vec(const float2 *p) { return __ldg(p); }
-    static __device__ __forceinline__ void out(float2 *p, float2 v) { __stcs(p, v); }
-};
+#include <algorithm>
+#include <stdlib.h>
+#include <vector>
 
-// acc[i] (+)= U v_i  (DAG = false)   or   acc[i] -= U^dag v_i  (DAG = true), i < T.
-// Column by column: for input colour b only U[.][b] (or, daggered, U[b][.]) and one complex per rhs are live, so the
-// register tile is 6 T accumulators + 6 link reals + the loads in flight.
-template <typename Real, int T, bool EXACT, bool DAG>
-__device__ __forceinline__ void hop(Real (&acc)[T][6], const typename CxT<Real>::type *__restrict__ U, size_t Vh,
-                                    const typename CxT<Real>::type *__restrict__ vin, int nvalid)
+static const int RING = 4; // shared-memory stages of 9 x 64 complex
+
+// ---------------------------------------------------------------- mbarrier / TMA (sm_90+ PTX, native on sm_100a)
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+// The consumer-side barrier operations and the shared-memory reads of the ring are volatile asm WITHOUT a memory
+// clobber: volatile asm statements keep their relative order, which is all the ring needs, while the compiler stays
+// free to move the global loads of the neighbour vectors across them (it must, to keep loads of the next hop in
+// flight while this hop waits for its links).
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)));
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_addr(bar)), "r"(parity));
+    } while (!ok);
+}
+__device__ __forceinline__ double2 lds_cx(const double2 *p)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(smem_addr(p)));
+    return v;
+}
+__device__ __forceinline__ float2 lds_cx(const float2 *p)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(smem_addr(p)));
+    return v;
+}
+__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_addr(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_addr(bar))
+                 : "memory");
+}
+
+template <int T> struct PipeDepth { static const int value = (3 * T) % 12 == 0 ? 12 : (3 * T) % 9 == 0 ? 9 : (3 * T) % 6 == 0 ? 6 : 3 * T; };
+
+// G rhs groups of T rhs each; blockDim = (64, G); MINB CTAs per SM
+template <typename Real, int T, int G, bool EXACT, int MINB>
+__global__ void __launch_bounds__(BKR_LINK_TILE *G, MINB)
+dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restrict__ wt, const int *__restrict__ tile_order,
+              const typename CxT<Real>::type *__restrict__ in, typename CxT<Real>::type *__restrict__ out,
+              const typename CxT<Real>::type *__restrict__ xp, Real a, int parity, const int *done)
 {
     typedef typename CxT<Real>::type Cx;
+    constexpr uint32_t STAGE_BYTES = 9 * BKR_LINK_TILE * sizeof(Cx);
+    constexpr int D = PipeDepth<T>::value; // neighbour loads in flight per thread; divides 3 T
+    __shared__ __align__(128) Cx stage[RING][9][BKR_LINK_TILE];
+    __shared__ __align__(8) uint64_t full[RING], empty[RING];
+    if (done && *done) return;
+    const int tid = threadIdx.y * BKR_LINK_TILE + threadIdx.x;
+    if (tid == 0) {
 #pragma unroll
-    for (int b = 0; b < 3; b++) {
-        Cx u[3]; // forward: column b of U;  backward: row b of U (conjugated below)
+        for (int s = 0; s < RING; s++) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], 2 * G); // one arrival per warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // CTA b visits the tiles tile_order[b], tile_order[b + grid], ...: at any time the CTAs of the grid work on a window
+    // of consecutive entries of the (L2-blocked) order
+    const int ntl = ((int)blockIdx.x < ntiles) ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int nstages = ntl * 16;
+    auto issue = [&](int st) { // producer: stage st = hop (st % 16) of this CTA's tile number st / 16
+        const int tile = tile_order[blockIdx.x + (st >> 4) * gridDim.x];
+        const Cx *src = wt + ((size_t)tile * 16 + (st & 15)) * 9 * BKR_LINK_TILE;
+        mbar_expect_tx(&full[st % RING], STAGE_BYTES);
+        tma_load_1d(&stage[st % RING][0][0], src, STAGE_BYTES, &full[st % RING]);
+    };
+    if (tid == 0)
+        for (int st = 0; st < RING && st < nstages; st++) issue(st);
+
+    const int j0 = threadIdx.y * T;
+    const int nvalid = N - j0;
+    const size_t Vh = g.Vh;
+    const Cx *vin = in + (size_t)j0 * 3 * Vh;
+
+    for (int k = 0; k < ntl; k++) {
+        const int e_raw = tile_order[blockIdx.x + k * gridDim.x] * BKR_LINK_TILE + threadIdx.x;
+        const bool valid = e_raw < g.Vh;
+        const int e = valid ? e_raw : g.Vh - 1; // tail tile: compute on a clamped site, store nothing
+        // coordinates of the output site (parity, e): lexicographic s = x + X(y + Y(z + Z t)), e = s / 2
+        int s = 2 * e;
+        int c[4];
+        const int x0 = s % g.X[0];
+        int r = s / g.X[0];
+        c[1] = r % g.X[1];
+        r /= g.X[1];
+        c[2] = r % g.X[2];
+        c[3] = r / g.X[2];
+        c[0] = x0 + ((c[1] + c[2] + c[3] + parity) & 1);
+        s = s - x0 + c[0];
+
+        Real acc[T][6];
 #pragma unroll
-        for (int a = 0; a < 3; a++) u[a] = LdSt<Real>::link(U + (DAG ? b * 3 + a : a * 3 + b) * Vh);
+        for (int i = 0; i < T; i++)
 #pragma unroll
-        for (int i = 0; i < T; i++) {
-            if (EXACT || i < nvalid) {
-                const Cx v = LdSt<Real>::vec(vin + (size_t)(i * 3 + b) * Vh);
+            for (int q = 0; q < 6; q++) acc[i][q] = (Real)0;
+
+        // Runtime loop over the 16 hops (fully unrolled they are ~100 KB of code and the warps stall on instruction
+        // fetch).  The neighbour-vector loads are software pipelined by hand: a register ring of D loads runs D
+        // (b, rhs) steps ahead of the FMAs, across hop boundaries, because one warp must keep ~D 512-byte loads in
+        // flight to cover L2/HBM latency at 12-16 warps per SM (measured: the compiler's own schedule kept ~2.4).
+        const int st0 = k * 16;
+        auto nbr = [&](int h) -> const Cx * {
+            const int mu = h >> 2, hop = (h & 2) ? 3 : 1;
+            const int cm = mu == 0 ? c[0] : mu == 1 ? c[1] : mu == 2 ? c[2] : c[3];
+            const int Xm = g.X[mu];
+            const int sm = mu == 0 ? 1 : mu == 1 ? g.X[0] : mu == 2 ? g.X[0] * g.X[1] : g.X[0] * g.X[1] * g.X[2];
+            int cn = (h & 1) ? cm - hop : cm + hop;
+            if (cn < 0) cn += Xm;
+            if (cn >= Xm) cn -= Xm;
+            return vin + ((s + (cn - cm) * sm) >> 1);
+        };
+        const Cx *vn = nbr(0);
+        Cx vbuf[D];
 #pragma unroll
-                for (int a = 0; a < 3; a++) {
-                    if (!DAG) { // + U_ab v_b
-                        acc[i][2 * a] = fma(u[a].x, v.x, acc[i][2 * a]);
-                        acc[i][2 * a] = fma(-u[a].y, v.y, acc[i][2 * a]);
-                        acc[i][2 * a + 1] = fma(u[a].x, v.y, acc[i][2 * a + 1]);
-                        acc[i][2 * a + 1] = fma(u[a].y, v.x, acc[i][2 * a + 1]);
-                    } else { // - conj(U_ba) v_b
-                        acc[i][2 * a] = fma(-u[a].x, v.x, acc[i][2 * a]);
-                        acc[i][2 * a] = fma(-u[a].y, v.y, acc[i][2 * a]);
-                        acc[i][2 * a + 1] = fma(-u[a].x, v.y, acc[i][2 * a + 1]);
-                        acc[i][2 * a + 1] = fma(u[a].y, v.x, acc[i][2 * a + 1]);
+        for (int n = 0; n < D; n++)
+            if (EXACT || (n % T) < nvalid) vbuf[n] = __ldg(vn + (size_t)((n % T) * 3 + n / T) * Vh);
+#pragma unroll 1
+        for (int h = 0; h < 16; h++) {
+            const int slot = h & (RING - 1);
+            const uint32_t ph = (h >> 2) & 1; // ((st0 + h) / RING) & 1 with RING = 4 and st0 / 4 even
+            // producer, one stage behind the consumers: refill the slot of the previous hop with the stage RING
+            // hops after it
+            if (tid == 0) {
+                const int prev = st0 + h - 1;
+                if (prev >= 0 && prev + RING < nstages) {
+                    mbar_wait(&empty[(h + RING - 1) & (RING - 1)], ((prev >> 2) & 1));
+                    issue(prev + RING);
+                }
+            }
+            const Cx *vnext = nbr(h < 15 ? h + 1 : 15);
+            mbar_wait(&full[slot], ph);
+            Cx u[3];
+#pragma unroll
+            for (int n = 0; n < 3 * T; n++) {
+                const int b = n / T, i = n % T;
+                if (i == 0) {
+#pragma unroll
+                    for (int aa = 0; aa < 3; aa++) u[aa] = lds_cx(&stage[slot][aa * 3 + b][threadIdx.x]);
+                }
+                const Cx v = vbuf[n % D];
+                const int m = n + D; // the step whose load takes this ring entry
+                if (m < 3 * T) {
+                    if (EXACT || (m % T) < nvalid) vbuf[n % D] = __ldg(vn + (size_t)((m % T) * 3 + m / T) * Vh);
+                } else if (h < 15) {
+                    const int m2 = m - 3 * T;
+                    if (EXACT || (m2 % T) < nvalid) vbuf[n % D] = __ldg(vnext + (size_t)((m2 % T) * 3 + m2 / T) * Vh);
+                }
+                if (EXACT || i < nvalid) {
+#pragma unroll
+                    for (int aa = 0; aa < 3; aa++) { // acc_a += W_ab v_b
+                        acc[i][2 * aa] = fma(u[aa].x, v.x, acc[i][2 * aa]);
+                        acc[i][2 * aa] = fma(-u[aa].y, v.y, acc[i][2 * aa]);
+                        acc[i][2 * aa + 1] = fma(u[aa].x, v.y, acc[i][2 * aa + 1]);
+                        acc[i][2 * aa + 1] = fma(u[aa].y, v.x, acc[i][2 * aa + 1]);
+                    }
+                }
+            }
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(&empty[slot]);
+            vn = vnext;
+        }
+
+        if (valid) {
+            Cx *vout = out + (size_t)j0 * 3 * Vh + e;
+            const Cx *vxp = xp ? xp + (size_t)j0 * 3 * Vh + e : nullptr;
+#pragma unroll
+            for (int i = 0; i < T; i++) {
+                if (EXACT || i < nvalid) {
+#pragma unroll
+                    for (int cc = 0; cc < 3; cc++) {
+                        Cx o;
+                        o.x = acc[i][2 * cc];
+                        o.y = acc[i][2 * cc + 1];
+                        if (vxp) {
+                            const Cx p = __ldg(vxp + (size_t)(i * 3 + cc) * Vh);
+                            o.x = fma(a, p.x, -o.x);
+                            o.y = fma(a, p.y, -o.y);
+                        }
+                        __stcs(vout + (size_t)(i * 3 + cc) * Vh, o);
                     }
                 }
             }
@@ -65,124 +230,112 @@ __device__ __forceinline__ void hop(Real (&acc)[T][6], const typename CxT<Real>:
     }
 }
 
-template <typename Real, int T, bool EXACT, int BS, int MINB>
-__global__ void __launch_bounds__(BS, MINB)
-dslash_kernel(Geom g, int parity, int N, const typename CxT<Real>::type *__restrict__ links,
-              const typename CxT<Real>::type *__restrict__ in, typename CxT<Real>::type *__restrict__ out,
-              const typename CxT<Real>::type *__restrict__ xp, Real a, const int *done)
+// ---------------------------------------------------------------- host: L2 blocking and dispatch
+
+// Order in which the link tiles (64 consecutive even-odd sites) are visited: (y, z) blocks outermost, then t, then
+// the sites of the block's time slice.  The block is the largest one whose 7-slice working set (t-3 .. t+3 of the
+// input block, N rhs) fits the L2 budget; cost = extra halo reads 6/YB + 6/ZB of the input per output site.
+static int build_tile_order(bkr_ctx *ctx, int N, int prec)
 {
-    typedef typename CxT<Real>::type Cx;
-    if (done && *done) return;
-    const int e = blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= g.Vh) return;
-    const int j0 = threadIdx.y * T;
-    const int nvalid = N - j0; // rhs this thread owns (>= 1 by construction of the launch; may be < T)
-    // coordinates of the output site (parity, e): lexicographic s = x + X(y + Y(z + Z t)), e = s / 2
-    int s = 2 * e;
-    int c[4];
-    const int x0 = s % g.X[0];
-    int r = s / g.X[0];
-    c[1] = r % g.X[1];
-    r /= g.X[1];
-    c[2] = r % g.X[2];
-    c[3] = r / g.X[2];
-    c[0] = x0 + ((c[1] + c[2] + c[3] + parity) & 1);
-    s = s - x0 + c[0];
-    const int stride[4] = {1, g.X[0], g.X[0] * g.X[1], g.X[0] * g.X[1] * g.X[2]};
-    const size_t Vh = g.Vh;
-
-    Real acc[T][6];
-#pragma unroll
-    for (int i = 0; i < T; i++)
-#pragma unroll
-        for (int k = 0; k < 6; k++) acc[i][k] = (Real)0;
-
-    const Cx *vin = in + (size_t)j0 * 3 * Vh;
-#pragma unroll
-    for (int mu = 0; mu < 4; mu++) {
-#pragma unroll
-        for (int type = 0; type < 2; type++) {
-            const int h = type ? 3 : 1;
-            int cf = c[mu] + h;
-            if (cf >= g.X[mu]) cf -= g.X[mu];
-            int cb = c[mu] - h;
-            if (cb < 0) cb += g.X[mu];
-            const int ef = (s + (cf - c[mu]) * stride[mu]) >> 1;
-            const int eb = (s + (cb - c[mu]) * stride[mu]) >> 1;
-            // forward: link leaving x (parity of x), vector at x + h mu
-            hop<Real, T, EXACT, false>(acc, links + (size_t)(((type * 4 + mu) * 2 + parity) * 9) * Vh + e, Vh, vin + ef,
-                                       nvalid);
-            // backward: link leaving x - h mu (opposite parity), daggered, vector at x - h mu
-            hop<Real, T, EXACT, true>(acc, links + (size_t)(((type * 4 + mu) * 2 + (1 - parity)) * 9) * Vh + eb, Vh,
-                                      vin + eb, nvalid);
-        }
-    }
-
-    Cx *vout = out + (size_t)j0 * 3 * Vh + e;
-    const Cx *vxp = xp ? xp + (size_t)j0 * 3 * Vh + e : nullptr;
-#pragma unroll
-    for (int i = 0; i < T; i++) {
-        if (EXACT || i < nvalid) {
-#pragma unroll
-            for (int cc = 0; cc < 3; cc++) {
-                Cx o;
-                o.x = acc[i][2 * cc];
-                o.y = acc[i][2 * cc + 1];
-                if (vxp) {
-                    const Cx p = LdSt<Real>::vec(vxp + (size_t)(i * 3 + cc) * Vh);
-                    o.x = fma(a, p.x, -o.x);
-                    o.y = fma(a, p.y, -o.y);
-                }
-                LdSt<Real>::out(vout + (size_t)(i * 3 + cc) * Vh, o);
+    const Geom &g = ctx->g;
+    const int Xh = g.X[0] / 2, Y = g.X[1], Z = g.X[2], Tt = g.X[3];
+    static const char *env = getenv("BKR_L2_BUDGET_MB");
+    const double budget = (env ? atof(env) : 48.0) * 1e6;
+    const double site_bytes = 3.0 * N * (prec == BKR_F64 ? 16 : 8);
+    int bestY = Y, bestZ = Z;
+    double best_cost = 1e30, best_ws = 0;
+    bool best_fits = false;
+    for (int yb = 1; yb <= Y; yb++) {
+        if (Y % yb) continue;
+        for (int zb = 1; zb <= Z; zb++) {
+            if (Z % zb) continue;
+            const double ws = 7.0 * Xh * yb * zb * site_bytes;
+            const bool fits = ws <= budget || Tt <= 7;
+            const double cost = (yb < Y ? 6.0 / yb : 0.0) + (zb < Z ? 6.0 / zb : 0.0);
+            bool better;
+            if (fits != best_fits) better = fits;
+            else if (fits) better = cost < best_cost - 1e-12 || (cost < best_cost + 1e-12 && ws > best_ws);
+            else better = ws < best_ws || best_ws == 0;
+            if (better) {
+                best_fits = fits;
+                best_cost = cost;
+                best_ws = ws;
+                bestY = yb;
+                bestZ = zb;
             }
         }
     }
+    const int key = bestY * 4096 + bestZ + 1;
+    if (ctx->tile_order && ctx->tile_order_key == key) return BKR_OK;
+    const int ntiles = link_tiles(g);
+    std::vector<std::pair<long long, int>> keys(ntiles);
+    const int nyb = Y / bestY;
+    for (int k = 0; k < ntiles; k++) {
+        const long long e0 = (long long)k * BKR_LINK_TILE;
+        const int y = (int)((e0 / Xh) % Y), z = (int)((e0 / ((long long)Xh * Y)) % Z), t = (int)(e0 / ((long long)Xh * Y * Z));
+        const long long blk = (long long)(z / bestZ) * nyb + y / bestY;
+        keys[k] = std::make_pair((blk * (Tt + 1) + t) * ((long long)ntiles + 1) + k, k);
+    }
+    std::sort(keys.begin(), keys.end());
+    std::vector<int> order(ntiles);
+    for (int k = 0; k < ntiles; k++) order[k] = keys[k].second;
+    if (!ctx->tile_order) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->tile_order, (size_t)ntiles * sizeof(int)));
+    // synchronous copy from pageable memory: the table is tiny and rebuilt only when the blocking changes
+    BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    BKR_CUDA(ctx, cudaMemcpy(ctx->tile_order, order.data(), (size_t)ntiles * sizeof(int), cudaMemcpyHostToDevice));
+    ctx->tile_order_key = key;
+    return BKR_OK;
 }
 
-// T rhs per thread, G = ceil(N / T) rhs groups per CTA, BS sites per CTA
-template <typename Real, int T, int BS, int MINB>
-static int launch_t(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
+template <typename Real, int T, int G, int MINB>
+static int launch_tg(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
     typedef typename CxT<Real>::type Cx;
-    const Cx *links = sizeof(Real) == 8 ? (const Cx *)ctx->links64 : (const Cx *)ctx->links32;
-    const int G = (N + T - 1) / T;
-    dim3 block(BS / G >= 32 ? (BS / G) / 32 * 32 : 32, G);
-    unsigned blocks = (unsigned)((ctx->g.Vh + block.x - 1) / block.x);
-    if (N % T == 0)
-        dslash_kernel<Real, T, true, BS, MINB><<<blocks, block, 0, ctx->stream>>>(ctx->g, parity, N, links, (const Cx *)in,
-                                                                                  (Cx *)out, (const Cx *)xp, (Real)a, done);
+    const int ntiles = link_tiles(ctx->g);
+    const Cx *wt = (sizeof(Real) == 8 ? (const Cx *)ctx->links64 : (const Cx *)ctx->links32) +
+                   (size_t)parity * ntiles * 16 * 9 * BKR_LINK_TILE;
+    dim3 block(BKR_LINK_TILE, G);
+    unsigned grid = (unsigned)std::min(ntiles, BKR_NUM_SMS * MINB);
+    if (N == T * G)
+        dslash_kernel<Real, T, G, true, MINB><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
+                                                                               (Cx *)out, (const Cx *)xp, (Real)a, parity, done);
     else
-        dslash_kernel<Real, T, false, BS, MINB><<<blocks, block, 0, ctx->stream>>>(ctx->g, parity, N, links, (const Cx *)in,
-                                                                                   (Cx *)out, (const Cx *)xp, (Real)a, done);
+        dslash_kernel<Real, T, G, false, MINB><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
+                                                                                (Cx *)out, (const Cx *)xp, (Real)a, parity, done);
     return bkr_check_launch(ctx);
 }
 
-// register tile T = ceil(N / ceil(N / 8)): N <= 8 -> T = N; 9..16 -> two groups; 17..24 -> three; 25..32 -> four
+// register tile T and rhs groups G:  N <= 8: one group (T = 1,2,3,4,6,8);  9..12: 2 x 6;  13..16: 2 x 8;
+// 17..24: 3 x 8;  25..32: 4 x 8
 template <typename Real>
 static int launch_n(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
-    const int G = (N + 7) / 8;
-    const int T = (N + G - 1) / G;
-    switch (T) {
-    case 1: return launch_t<Real, 1, 128, 4>(ctx, parity, N, in, out, xp, a, done);
-    case 2: return launch_t<Real, 2, 128, 4>(ctx, parity, N, in, out, xp, a, done);
-    case 3: return launch_t<Real, 3, 128, 4>(ctx, parity, N, in, out, xp, a, done);
-    case 4: return launch_t<Real, 4, 128, 4>(ctx, parity, N, in, out, xp, a, done);
-    case 5: return launch_t<Real, 5, 128, 3>(ctx, parity, N, in, out, xp, a, done);
-    case 6: return launch_t<Real, 6, 128, 3>(ctx, parity, N, in, out, xp, a, done);
-    case 7: return launch_t<Real, 7, 128, 3>(ctx, parity, N, in, out, xp, a, done);
-    case 8: return launch_t<Real, 8, 128, 3>(ctx, parity, N, in, out, xp, a, done);
+#define GO(T_, G_, M_) return launch_tg<Real, T_, G_, M_>(ctx, parity, N, in, out, xp, a, done)
+    static const char *env = getenv("BKR_DSLASH_T4"); // tuning hook: 4 rhs per thread, more groups
+    if (env && atoi(env)) {
+        if (N > 4 && N <= 8) GO(4, 2, 4);
+        if (N > 8 && N <= 12) GO(4, 3, 3);
+        if (N > 12 && N <= 16) GO(4, 4, 2);
     }
+    if (N == 1) GO(1, 1, 6);
+    if (N == 2) GO(2, 1, 6);
+    if (N == 3) GO(3, 1, 6);
+    if (N == 4) GO(4, 1, 6);
+    if (N <= 6) GO(6, 1, 6);
+    if (N <= 8) GO(8, 1, 6);
+    if (N <= 12) GO(6, 2, 3);
+    if (N <= 16) GO(8, 2, 3);
+    if (N <= 24) GO(8, 3, 2);
+    if (N <= 32) GO(8, 4, 1);
+#undef GO
     return BKR_EINVAL;
 }
 
 int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp, double a,
                   const int *done)
 {
-    if (prec == BKR_F64) {
-        if (!ctx->links64) return BKR_ENOLINKS;
-        return launch_n<double>(ctx, out_parity, N, in, out, xp, a, done);
-    }
-    if (!ctx->links32) return BKR_ENOLINKS;
+    if (!(prec == BKR_F64 ? (void *)ctx->links64 : (void *)ctx->links32)) return BKR_ENOLINKS;
+    BKR_TRY(build_tile_order(ctx, N, prec));
+    if (prec == BKR_F64) return launch_n<double>(ctx, out_parity, N, in, out, xp, a, done);
     return launch_n<float>(ctx, out_parity, N, in, out, xp, a, done);
 }

@@ -6,44 +6,74 @@
 //                                  vector the three colour planes are SoA over the even-odd site index, so a
 //                                  warp of 32 consecutive sites (stencil) or rows (block BLAS) reads 512
 //                                  contiguous bytes per instruction in fp64.
-//   native links  L[d][el][e]    : d = (type*4 + mu)*2 + parity, el = 3*row + col; complex SoA over sites, so
-//                                  the lanes of a warp that work on different sites read contiguous 16 B
-//                                  (fp64) / 8 B (fp32) pieces and lanes on the same site broadcast.
+//   native links  Wt[p][tile][h][el][lane] : gather form, tile-major (see pack_links_kernel below).
 #include "common.cuh"
 
-__global__ void pack_links_kernel(Geom g, const double2 *__restrict__ fat, const double2 *__restrict__ lng,
+// Gather-form links.  For the output site x of parity p (even-odd index e) and hop h = ((mu*2 + type)*2 + dir)
+// (type 0 fat / 1 long, hop length 1 / 3; dir 0 forward / 1 backward) the stencil needs the matrix
+//     W_h(x) = U_mu(x)                (forward)         W_h(x) = - U_mu(x - hop mu)^dagger   (backward)
+// so that (D in)(x) = sum_h W_h(x) in(nbr_h(x))  (eq. 2).  Storing W per output site makes the
+// whole link stream of a tile of BKR_LINK_TILE consecutive sites ONE contiguous chunk
+//     Wt[p][tile][h][el][lane],   el = 3*row + col,  lane = e % BKR_LINK_TILE,
+// which the stencil kernel streams with 1-D TMA bulk copies, one per hop.  Bytes read per call are unchanged
+// (16 matrices per output site); storage is twice the canonical links (each U appears as a forward and as a
+// backward copy).
+__global__ void pack_links_kernel(Geom g, int ntiles, const double2 *__restrict__ fat, const double2 *__restrict__ lng,
                                   double2 *__restrict__ out64, float2 *__restrict__ out32)
 {
-    // one thread per (type, mu, site, el)
-    size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    size_t total = (size_t)2 * 4 * g.V * 9;
-    if (tid >= total) return;
-    int el = (int)(tid % 9);
-    size_t r = tid / 9;
-    int s = (int)(r % g.V);
-    r /= g.V;
-    int mu = (int)(r % 4);
-    int type = (int)(r / 4);
-    int x = s % g.X[0];
-    int q = s / g.X[0];
-    int y = q % g.X[1];
-    q /= g.X[1];
-    int z = q % g.X[2];
-    int t = q / g.X[2];
-    int parity = (x + y + z + t) & 1;
-    int e = s >> 1;
-    const double2 *src = (type == 0 ? fat : lng) + ((size_t)mu * g.V + s) * 9 + el;
-    double2 u = *src;
-    size_t o = ((size_t)(((type * 4 + mu) * 2 + parity) * 9 + el)) * g.Vh + e;
-    out64[o] = u;
-    if (out32) out32[o] = make_float2((float)u.x, (float)u.y);
+    // one thread per (parity, e, h)
+    const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t padded = (size_t)ntiles * BKR_LINK_TILE;
+    if (tid >= 2 * padded * 16) return;
+    const int h = (int)(tid % 16);
+    const size_t r = tid / 16;
+    const int e = (int)(r % padded);
+    const int parity = (int)(r / padded);
+    const int mu = h >> 2, type = (h >> 1) & 1, dir = h & 1;
+    const size_t base = ((((size_t)parity * ntiles + e / BKR_LINK_TILE) * 16 + h) * 9) * BKR_LINK_TILE + e % BKR_LINK_TILE;
+    double2 w[9];
+    if (e < g.Vh) {
+        int s = 2 * e;
+        int c[4];
+        const int x0 = s % g.X[0];
+        int q = s / g.X[0];
+        c[1] = q % g.X[1];
+        q /= g.X[1];
+        c[2] = q % g.X[2];
+        c[3] = q / g.X[2];
+        c[0] = x0 + ((c[1] + c[2] + c[3] + parity) & 1);
+        s = s - x0 + c[0];
+        const int stride[4] = {1, g.X[0], g.X[0] * g.X[1], g.X[0] * g.X[1] * g.X[2]};
+        const double2 *src = (type == 0 ? fat : lng) + (size_t)mu * g.V * 9;
+        if (dir == 0) {
+            for (int el = 0; el < 9; el++) w[el] = src[(size_t)s * 9 + el];
+        } else {
+            const int hop = type ? 3 : 1;
+            int cb = c[mu] - hop;
+            if (cb < 0) cb += g.X[mu];
+            const int sb = s + (cb - c[mu]) * stride[mu];
+            for (int a = 0; a < 3; a++)
+                for (int b = 0; b < 3; b++) {
+                    const double2 u = src[(size_t)sb * 9 + b * 3 + a];
+                    w[a * 3 + b] = make_double2(-u.x, u.y); // -conj(U_ba)
+                }
+        }
+    } else {
+        for (int el = 0; el < 9; el++) w[el] = make_double2(0.0, 0.0);
+    }
+    for (int el = 0; el < 9; el++) {
+        const size_t o = base + (size_t)el * BKR_LINK_TILE;
+        if (out64) out64[o] = w[el];
+        if (out32) out32[o] = make_float2((float)w[el].x, (float)w[el].y);
+    }
 }
 
 int launch_pack_links(bkr_ctx *ctx, const double2 *fat, const double2 *lng, double2 *out64, float2 *out32)
 {
-    size_t total = (size_t)2 * 4 * ctx->g.V * 9;
+    const int ntiles = link_tiles(ctx->g);
+    size_t total = (size_t)2 * ntiles * BKR_LINK_TILE * 16;
     unsigned blocks = (unsigned)((total + 255) / 256);
-    pack_links_kernel<<<blocks, 256, 0, ctx->stream>>>(ctx->g, fat, lng, out64, out32);
+    pack_links_kernel<<<blocks, 256, 0, ctx->stream>>>(ctx->g, ntiles, fat, lng, out64, out32);
     return bkr_check_launch(ctx);
 }
 
