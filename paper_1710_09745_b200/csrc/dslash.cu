@@ -73,19 +73,34 @@ __device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t
                  "l"(src), "r"(bytes), "r"(smem_addr(bar))
                  : "memory");
 }
+// the same with an L2 eviction policy: the links are used once per call, so they should not displace the vectors
+__device__ __forceinline__ void tma_load_1d_hint(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+                     smem_addr(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_addr(bar)), "l"(pol)
+                 : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_first()
+{
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+
 
 template <int T> struct PipeDepth { static const int value = (3 * T) % 12 == 0 ? 12 : (3 * T) % 9 == 0 ? 9 : (3 * T) % 6 == 0 ? 6 : 3 * T; };
 
 // G rhs groups of T rhs each; blockDim = (64, G); MINB CTAs per SM
-template <typename Real, int T, int G, bool EXACT, int MINB>
+template <typename Real, int T, int G, bool EXACT, int MINB, int DD>
 __global__ void __launch_bounds__(BKR_LINK_TILE *G, MINB)
 dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restrict__ wt, const int *__restrict__ tile_order,
               const typename CxT<Real>::type *__restrict__ in, typename CxT<Real>::type *__restrict__ out,
-              const typename CxT<Real>::type *__restrict__ xp, Real a, int parity, const int *done)
+              const typename CxT<Real>::type *__restrict__ xp, Real a, int parity, const int *done, int opts)
 {
     typedef typename CxT<Real>::type Cx;
     constexpr uint32_t STAGE_BYTES = 9 * BKR_LINK_TILE * sizeof(Cx);
-    constexpr int D = PipeDepth<T>::value; // neighbour loads in flight per thread; divides 3 T
+    constexpr int D = DD > 0 ? DD : PipeDepth<T>::value; // neighbour loads in flight per thread; divides 3 T
     __shared__ __align__(128) Cx stage[RING][9][BKR_LINK_TILE];
     __shared__ __align__(8) uint64_t full[RING], empty[RING];
     if (done && *done) return;
@@ -104,11 +119,13 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
     // of consecutive entries of the (L2-blocked) order
     const int ntl = ((int)blockIdx.x < ntiles) ? (ntiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
     const int nstages = ntl * 16;
+    const uint64_t pol = policy_evict_first();
     auto issue = [&](int st) { // producer: stage st = hop (st % 16) of this CTA's tile number st / 16
         const int tile = tile_order[blockIdx.x + (st >> 4) * gridDim.x];
         const Cx *src = wt + ((size_t)tile * 16 + (st & 15)) * 9 * BKR_LINK_TILE;
         mbar_expect_tx(&full[st % RING], STAGE_BYTES);
-        tma_load_1d(&stage[st % RING][0][0], src, STAGE_BYTES, &full[st % RING]);
+        if (opts & 1) tma_load_1d(&stage[st % RING][0][0], src, STAGE_BYTES, &full[st % RING]);
+        else tma_load_1d_hint(&stage[st % RING][0][0], src, STAGE_BYTES, &full[st % RING], pol);
     };
     if (tid == 0)
         for (int st = 0; st < RING && st < nstages; st++) issue(st);
@@ -287,21 +304,23 @@ static int build_tile_order(bkr_ctx *ctx, int N, int prec)
     return BKR_OK;
 }
 
-template <typename Real, int T, int G, int MINB>
+template <typename Real, int T, int G, int MINB, int DD = 0>
 static int launch_tg(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
     typedef typename CxT<Real>::type Cx;
     const int ntiles = link_tiles(ctx->g);
     const Cx *wt = (sizeof(Real) == 8 ? (const Cx *)ctx->links64 : (const Cx *)ctx->links32) +
                    (size_t)parity * ntiles * 16 * 9 * BKR_LINK_TILE;
+    static const char *oenv = getenv("BKR_DSLASH_OPTS");
+    const int opts = oenv ? atoi(oenv) : 0;
     dim3 block(BKR_LINK_TILE, G);
     unsigned grid = (unsigned)std::min(ntiles, BKR_NUM_SMS * MINB);
     if (N == T * G)
-        dslash_kernel<Real, T, G, true, MINB><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
-                                                                               (Cx *)out, (const Cx *)xp, (Real)a, parity, done);
+        dslash_kernel<Real, T, G, true, MINB, DD><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
+                                                                               (Cx *)out, (const Cx *)xp, (Real)a, parity, done, opts);
     else
-        dslash_kernel<Real, T, G, false, MINB><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
-                                                                                (Cx *)out, (const Cx *)xp, (Real)a, parity, done);
+        dslash_kernel<Real, T, G, false, MINB, DD><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
+                                                                                (Cx *)out, (const Cx *)xp, (Real)a, parity, done, opts);
     return bkr_check_launch(ctx);
 }
 
@@ -311,11 +330,33 @@ template <typename Real>
 static int launch_n(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
 #define GO(T_, G_, M_) return launch_tg<Real, T_, G_, M_>(ctx, parity, N, in, out, xp, a, done)
-    static const char *env = getenv("BKR_DSLASH_T4"); // tuning hook: 4 rhs per thread, more groups
-    if (env && atoi(env)) {
-        if (N > 4 && N <= 8) GO(4, 2, 4);
-        if (N > 8 && N <= 12) GO(4, 3, 3);
-        if (N > 12 && N <= 16) GO(4, 4, 2);
+    static const char *cfg = getenv("BKR_DSLASH_CFG"); // tuning hook: "T,G,MINB,D"
+    if (cfg) {
+        int t = 0, gg = 0, mb = 0, dd = 0;
+        sscanf(cfg, "%d,%d,%d,%d", &t, &gg, &mb, &dd);
+        if (N <= t * gg) {
+#define TRY(T_, G_, M_, D_) if (t == T_ && gg == G_ && mb == M_ && dd == D_) return launch_tg<Real, T_, G_, M_, D_>(ctx, parity, N, in, out, xp, a, done)
+            TRY(8, 2, 3, 6); TRY(8, 2, 3, 4); TRY(8, 2, 2, 12); TRY(8, 2, 2, 8); TRY(8, 2, 2, 24); TRY(4, 4, 2, 6); TRY(4, 4, 2, 4); TRY(4, 4, 2, 12);
+            TRY(6, 3, 2, 9); TRY(6, 3, 2, 6); TRY(8, 1, 4, 12); TRY(8, 1, 4, 8); TRY(8, 1, 6, 6); TRY(4, 2, 4, 6); TRY(4, 2, 4, 4); TRY(4, 2, 4, 12); TRY(4, 2, 3, 12);
+            TRY(8, 4, 1, 12); TRY(8, 4, 1, 24); TRY(8, 3, 1, 12); TRY(4, 8, 1, 6); TRY(4, 6, 1, 6); TRY(4, 6, 1, 12); TRY(4, 8, 1, 12);
+#undef TRY
+        }
+    }
+    // Register budget decides the shape (ptxas -v: the fp64 T = 8 thread needs ~190 registers for 48 accumulators, the
+    // 12-deep load ring and the link column; under a 168-register cap it spills ~0.5 KB per thread, and ncu showed the
+    // spill traffic, not the stencil, filling the LSU).  fp64: at most 2 CTAs of 128 threads (or 4 of 64) per SM.
+    if (sizeof(Real) == 8) {
+        if (N == 1) GO(1, 1, 6);
+        if (N == 2) GO(2, 1, 6);
+        if (N == 3) GO(3, 1, 6);
+        if (N == 4) GO(4, 1, 6);
+        if (N <= 6) GO(6, 1, 6);
+        if (N <= 8) return launch_tg<Real, 8, 1, 4, 12>(ctx, parity, N, in, out, xp, a, done);
+        if (N <= 12) GO(6, 2, 3);
+        if (N <= 16) return launch_tg<Real, 8, 2, 2, 12>(ctx, parity, N, in, out, xp, a, done);
+        if (N <= 24) return launch_tg<Real, 4, 6, 1, 12>(ctx, parity, N, in, out, xp, a, done);
+        if (N <= 32) return launch_tg<Real, 8, 4, 1, 12>(ctx, parity, N, in, out, xp, a, done);
+        return BKR_EINVAL;
     }
     if (N == 1) GO(1, 1, 6);
     if (N == 2) GO(2, 1, 6);
