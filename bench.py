@@ -86,11 +86,18 @@ class ClockSampler:
 
     def __init__(self, index):
         self.rows, self.proc, self.index = [], None, index
+        self.t0 = self.t1 = None
+
+    def mark_begin(self):
+        self.t0 = time.time()
+
+    def mark_end(self):
+        self.t1 = time.time()
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -99,27 +106,32 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append([time.time()] + [c.strip() for c in line.split(",")])
 
     def stop(self):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
         self.t.join(timeout=2)
-        sm, mx, reasons = [], None, set()
+        sm, mx, reasons, power = [], None, set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
+        # samples taken between mark_begin() and mark_end() (the timed steps and the per-kernel timing loops: the GPU
+        # is busy throughout); a sample is stamped when its line arrives
+        inside = [r for r in self.rows if self.t0 is None or (self.t0 <= r[0] <= (self.t1 or 1e30))]
+        for r in inside:
             try:
-                sm.append(float(r[0]))
-                mx = float(r[1])
+                sm.append(float(r[1]))
+                mx = float(r[2])
+                power.append(float(r[3]))
             except (ValueError, IndexError):
                 continue
-            for n, v in zip(names, r[3:7]):
+            for n, v in zip(names, r[4:8]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
         sm.sort()
         return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
-                "samples": len(sm)}
+                "sm_mhz_min": sm[0] if sm else None, "samples": len(sm), "power_w_max": max(power) if power else None,
+                "window": "timed steps + per-kernel timing loops"}
 
 
 # ---------------------------------------------------------------- timing helpers
@@ -136,6 +148,28 @@ def time_loop(torch, fn, reps, warmup):
     e1.record()
     torch.cuda.synchronize()
     return e0.elapsed_time(e1) / reps
+
+
+SM_COUNT, SM_MAX_MHZ = 148, 1965.0
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
+# capture of this same bench command (profiles/r1_ncu_summary.md); None where no capture exists.
+NCU_TRAFFIC = {("cfg3", 16, "f64"): 4.843805e9 + 0.790890e9}
+
+
+def alu_peak_gflops(fp64):
+    """FMA-pipe peak DESIGN.md section 6.4 derives from the guide's unit counts: 148 SMs x 64 FP64 (128 FP32) lanes x
+    2 flop x 1.965 GHz.  The DMMA path of the multi-BLAS kernels has the same FP64 peak (measured 36.8 TFLOP/s)."""
+    return SM_COUNT * (64 if fp64 else 128) * 2 * SM_MAX_MHZ * 1e-3
+
+
+def roofline_entry(ms, by, fl, hbm, fp64_math):
+    """GB/s, GFLOPS, fraction of the HBM roofline, and fraction of max(bytes / BW, flops / ALU peak) with the binding
+    term named."""
+    t_hbm = by / hbm * 1e-6      # ms
+    t_alu = fl / alu_peak_gflops(fp64_math) * 1e-6
+    return {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": t_hbm / ms,
+            "frac_roofline": max(t_hbm, t_alu) / ms, "binding": "hbm" if t_hbm >= t_alu else "alu"}
 
 
 def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
@@ -158,28 +192,35 @@ def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
         ctx.dslash(i[0] & 1, N, s, d, prec)
     ms = time_loop(torch, f_dslash, reps, warmup)
     by, fl = bytes_dslash(dims, N, w), flops_dslash(dims, N)
-    out["dslash"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+    out["dslash"] = roofline_entry(ms, by, fl, hbm, prec == binding.F64)
 
     def f_gram2():
         s, d = rot()
         ctx.gram(N, s, d, hermitian=False, prec=prec, out=K)
     ms = time_loop(torch, f_gram2, reps, warmup)
     by, fl = 2 * block_bytes(dims, N, w), 8 * L * N * N
-    out["gram_xy"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+    out["gram_xy"] = roofline_entry(ms, by, fl, hbm, True)
+
+    def f_gram2h():
+        s, d = rot()
+        ctx.gram(N, s, d, hermitian=True, prec=prec, out=K)
+    ms = time_loop(torch, f_gram2h, reps, warmup)
+    by, fl = 2 * block_bytes(dims, N, w), 4 * L * N * (N + 1)
+    out["gram_xy_herm"] = roofline_entry(ms, by, fl, hbm, True)
 
     def f_gram1():
         s, _ = rot()
         ctx.gram(N, s, s, hermitian=True, prec=prec, out=K)
     ms = time_loop(torch, f_gram1, reps, warmup)
     by, fl = block_bytes(dims, N, w), 4 * L * N * (N + 1)
-    out["gram_xx"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+    out["gram_xx"] = roofline_entry(ms, by, fl, hbm, True)
 
     def f_axpy():
         s, d = rot()
         ctx.block_axpy(N, a, s, d, prec)
     ms = time_loop(torch, f_axpy, reps, warmup)
     by, fl = 3 * block_bytes(dims, N, w), 8 * L * N * N
-    out["block_axpy"] = {"ms": ms, "GBps": by / ms * 1e-6, "GFLOPS": fl / ms * 1e-6, "frac_hbm": by / ms * 1e-6 / hbm}
+    out["block_axpy"] = roofline_entry(ms, by, fl, hbm, True)
     return out
 
 
@@ -275,12 +316,13 @@ def run_bkr(args):
     ctx.load_links(fat, lng, also_f32=True)
     del fat, lng
     torch.cuda.empty_cache()
+    sampler = ClockSampler(local)
+    sampler.start()  # nvidia-smi takes a while to start: launched before the warm-up, windowed to the timed region
 
     # ---- timed region: K iterations after W warm-up iterations, device-resident
     launches_w = ctx.bench_iterations(mass, B, args.warmup, prec)
     torch.cuda.synchronize()
-    sampler = ClockSampler(local)
-    sampler.start()
+    sampler.mark_begin()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if dist:
         dist.barrier()
@@ -301,7 +343,8 @@ def run_bkr(args):
     value = world * by_iter / ms_step * 1e-6
 
     # ---- the dominant kernel alone (multi-rhs Dslash), and the multi-BLAS kernels, at this N
-    kern = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=max(10, args.steps), warmup=3, hbm=hbm)
+    kern = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=max(50, args.steps), warmup=3, hbm=hbm)
+    sampler.mark_end()
     clocks = sampler.stop()
 
     # ---- end to end through the host-buffer entry point (copies inside the timed region)
@@ -358,7 +401,9 @@ def run_bkr(args):
         "frac_hbm_iteration": value / world / hbm,
         "GFLOPS_iteration": world * flops_iteration(dims, N) / ms_step * 1e-6,
         "roofline": {"bound": "hbm", "kernel": "dslash_kernel (multi-rhs Dslash, one parity, N=%d)" % N,
-                     "achieved": d["GBps"], "peak": hbm, "unit": "GB/s", "frac": d["GBps"] / hbm, "traffic": None,
+                     "achieved": d["GBps"], "peak": hbm, "unit": "GB/s", "frac": d["GBps"] / hbm,
+                     "traffic": NCU_TRAFFIC.get((args.workload, N, "f64" if prec == binding.F64 else "f32")),
+                     "frac_roofline": d["frac_roofline"], "binding": d["binding"],
                      "peak_source": peak_src, "ms_per_launch": d["ms"],
                      "algorithmic_bytes_per_launch": bytes_dslash(dims, N, w), "GFLOPS": d["GFLOPS"]},
         "kernels": kern,
@@ -412,7 +457,7 @@ def run_sweep(args):
             k = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=args.steps, warmup=3, hbm=hbm)
             row = {"sweep": name, "dtype": pname, "N": N}
             for kn, v in k.items():
-                row[kn] = {a: round(b, 4) for a, b in v.items()}
+                row[kn] = {a: (round(b, 4) if isinstance(b, float) else b) for a, b in v.items()}
             print(json.dumps(row), flush=True)
     return 0
 

@@ -19,80 +19,20 @@
 //    block needs for its t +- 1, +- 3 hops stay L2-resident (tile_order, built on the host below).
 //  * Per site and rhs: 16 x 36 = 576 FMAs (1152 flop; the paper counts 1146).
 #include "common.cuh"
+#include "tma.cuh"
 
 #include <algorithm>
 #include <stdlib.h>
 #include <vector>
 
-static const int RING = 4; // shared-memory stages of 9 x 64 complex
-
-// ---------------------------------------------------------------- mbarrier / TMA (sm_90+ PTX, native on sm_100a)
-__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
-}
-// The consumer-side barrier operations and the shared-memory reads of the ring are volatile asm WITHOUT a memory
-// clobber: volatile asm statements keep their relative order, which is all the ring needs, while the compiler stays
-// free to move the global loads of the neighbour vectors across them (it must, to keep loads of the next hop in
-// flight while this hop waits for its links).
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)));
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(smem_addr(bar)), "r"(parity));
-    } while (!ok);
-}
-__device__ __forceinline__ double2 lds_cx(const double2 *p)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(smem_addr(p)));
-    return v;
-}
-__device__ __forceinline__ float2 lds_cx(const float2 *p)
-{
-    float2 v;
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(smem_addr(p)));
-    return v;
-}
-__device__ __forceinline__ void tma_load_1d(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_addr(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_addr(bar))
-                 : "memory");
-}
-// the same with an L2 eviction policy: the links are used once per call, so they should not displace the vectors
-__device__ __forceinline__ void tma_load_1d_hint(void *dst, const void *src, uint32_t bytes, uint64_t *bar, uint64_t pol)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
-                     smem_addr(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_addr(bar)), "l"(pol)
-                 : "memory");
-}
-__device__ __forceinline__ uint64_t policy_evict_first()
-{
-    uint64_t pol;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    return pol;
-}
-
+// shared-memory stages of 9 x 64 complex per CTA (template parameter RG of the kernel): the link stream has to be
+// requested far enough ahead to cover a loaded HBM round trip (ncu: with 4 stages = 3 hops ahead, 12 % of all warp
+// time was spent in the try_wait of the "full" barrier), so the ring is as deep as the CTAs-per-SM budget allows.
 
 template <int T> struct PipeDepth { static const int value = (3 * T) % 12 == 0 ? 12 : (3 * T) % 9 == 0 ? 9 : (3 * T) % 6 == 0 ? 6 : 3 * T; };
 
-// G rhs groups of T rhs each; blockDim = (64, G); MINB CTAs per SM
-template <typename Real, int T, int G, bool EXACT, int MINB, int DD>
+// G rhs groups of T rhs each; blockDim = (64, G); MINB CTAs per SM; RG ring stages (a power of two <= 16)
+template <typename Real, int T, int G, bool EXACT, int MINB, int DD, int RG>
 __global__ void __launch_bounds__(BKR_LINK_TILE *G, MINB)
 dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restrict__ wt, const int *__restrict__ tile_order,
               const typename CxT<Real>::type *__restrict__ in, typename CxT<Real>::type *__restrict__ out,
@@ -101,8 +41,12 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
     typedef typename CxT<Real>::type Cx;
     constexpr uint32_t STAGE_BYTES = 9 * BKR_LINK_TILE * sizeof(Cx);
     constexpr int D = DD > 0 ? DD : PipeDepth<T>::value; // neighbour loads in flight per thread; divides 3 T
-    __shared__ __align__(128) Cx stage[RING][9][BKR_LINK_TILE];
-    __shared__ __align__(8) uint64_t full[RING], empty[RING];
+    constexpr int RING = RG;
+    static_assert(RG == 2 || RG == 4 || RG == 8 || RG == 16, "ring depth must divide the 16 hops of a tile");
+    extern __shared__ __align__(128) unsigned char dsm[];
+    Cx(*stage)[9][BKR_LINK_TILE] = reinterpret_cast<Cx(*)[9][BKR_LINK_TILE]>(dsm);
+    uint64_t *full = reinterpret_cast<uint64_t *>(dsm + (size_t)RING * STAGE_BYTES);
+    uint64_t *empty = full + RING;
     if (done && *done) return;
     const int tid = threadIdx.y * BKR_LINK_TILE + threadIdx.x;
     if (tid == 0) {
@@ -165,28 +109,36 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
         auto nbr = [&](int h) -> const Cx * {
             const int mu = h >> 2, hop = (h & 2) ? 3 : 1;
             const int cm = mu == 0 ? c[0] : mu == 1 ? c[1] : mu == 2 ? c[2] : c[3];
-            const int Xm = g.X[mu];
+            // select chains, not g.X[mu]: an indexed constant load is a scoreboarded (variable-latency) load, and the
+            // in-order warp waited for it at the top of every hop (ncu source page: 8 % of all warp time)
+            const int Xm = mu == 0 ? g.X[0] : mu == 1 ? g.X[1] : mu == 2 ? g.X[2] : g.X[3];
             const int sm = mu == 0 ? 1 : mu == 1 ? g.X[0] : mu == 2 ? g.X[0] * g.X[1] : g.X[0] * g.X[1] * g.X[2];
             int cn = (h & 1) ? cm - hop : cm + hop;
             if (cn < 0) cn += Xm;
             if (cn >= Xm) cn -= Xm;
             return vin + ((s + (cn - cm) * sm) >> 1);
         };
-        const Cx *vn = nbr(0);
+        // One running pointer walks over the neighbour loads in consumption order n = b T + i (address index
+        // (3 i + b) Vh): += 3 Vh inside a colour b, += (1 - 3 (T - 1)) Vh at a colour change, = base of the next hop
+        // after the last load of this one.  (Per-load base + k Vh addresses cost ptxas ~90 live registers.)
+        const ptrdiff_t d_rhs = 3 * (ptrdiff_t)Vh, d_col = (1 - 3 * (T - 1)) * (ptrdiff_t)Vh;
+        const Cx *pl = nbr(0);
         Cx vbuf[D];
 #pragma unroll
-        for (int n = 0; n < D; n++)
-            if (EXACT || (n % T) < nvalid) vbuf[n] = __ldg(vn + (size_t)((n % T) * 3 + n / T) * Vh);
+        for (int n = 0; n < D; n++) {
+            if (EXACT || (n % T) < nvalid) vbuf[n] = __ldg(pl);
+            pl += ((n + 1) % T) ? d_rhs : d_col;
+        }
 #pragma unroll 1
         for (int h = 0; h < 16; h++) {
-            const int slot = h & (RING - 1);
-            const uint32_t ph = (h >> 2) & 1; // ((st0 + h) / RING) & 1 with RING = 4 and st0 / 4 even
+            const int slot = h & (RING - 1);      // (st0 + h) % RING: st0 = 16 k is a multiple of RING
+            const uint32_t ph = ((st0 + h) / RING) & 1;
             // producer, one stage behind the consumers: refill the slot of the previous hop with the stage RING
             // hops after it
             if (tid == 0) {
                 const int prev = st0 + h - 1;
                 if (prev >= 0 && prev + RING < nstages) {
-                    mbar_wait(&empty[(h + RING - 1) & (RING - 1)], ((prev >> 2) & 1));
+                    mbar_wait(&empty[prev & (RING - 1)], ((prev / RING) & 1));
                     issue(prev + RING);
                 }
             }
@@ -201,12 +153,11 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
                     for (int aa = 0; aa < 3; aa++) u[aa] = lds_cx(&stage[slot][aa * 3 + b][threadIdx.x]);
                 }
                 const Cx v = vbuf[n % D];
-                const int m = n + D; // the step whose load takes this ring entry
-                if (m < 3 * T) {
-                    if (EXACT || (m % T) < nvalid) vbuf[n % D] = __ldg(vn + (size_t)((m % T) * 3 + m / T) * Vh);
-                } else if (h < 15) {
-                    const int m2 = m - 3 * T;
-                    if (EXACT || (m2 % T) < nvalid) vbuf[n % D] = __ldg(vnext + (size_t)((m2 % T) * 3 + m2 / T) * Vh);
+                const int m = n + D; // the step whose load takes this ring entry (m >= 3 T: step m - 3 T of the next hop)
+                if (m == 3 * T) pl = vnext;
+                if (m < 3 * T || h < 15) {
+                    if (EXACT || (m % T) < nvalid) vbuf[n % D] = __ldg(pl);
+                    pl += ((m + 1) % T) ? d_rhs : d_col;
                 }
                 if (EXACT || i < nvalid) {
 #pragma unroll
@@ -220,7 +171,6 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
             }
             __syncwarp();
             if ((tid & 31) == 0) mbar_arrive(&empty[slot]);
-            vn = vnext;
         }
 
         if (valid) {
@@ -304,10 +254,19 @@ static int build_tile_order(bkr_ctx *ctx, int N, int prec)
     return BKR_OK;
 }
 
-template <typename Real, int T, int G, int MINB, int DD = 0>
+// default ring depth: as many 9 x 64-complex stages as leave about 100 KB of the SM's 256 KB for L1 (x-direction
+// neighbour reuse lives there)
+template <typename Real, int MINB> struct RingDepth {
+    static const int per_cta = 150 * 1024 / MINB / (9 * BKR_LINK_TILE * 2 * (int)sizeof(Real));
+    static const int value = per_cta >= 16 ? 16 : per_cta >= 8 ? 8 : per_cta >= 4 ? 4 : 2;
+};
+
+template <typename Real, int T, int G, int MINB, int DD = 0, int RGG = 0>
 static int launch_tg(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
     typedef typename CxT<Real>::type Cx;
+    constexpr int RG = RGG > 0 ? RGG : RingDepth<Real, MINB>::value;
+    constexpr size_t SMEM = (size_t)RG * 9 * BKR_LINK_TILE * sizeof(Cx) + 2 * RG * sizeof(uint64_t);
     const int ntiles = link_tiles(ctx->g);
     const Cx *wt = (sizeof(Real) == 8 ? (const Cx *)ctx->links64 : (const Cx *)ctx->links32) +
                    (size_t)parity * ntiles * 16 * 9 * BKR_LINK_TILE;
@@ -315,12 +274,20 @@ static int launch_tg(bkr_ctx *ctx, int parity, int N, const void *in, void *out,
     const int opts = oenv ? atoi(oenv) : 0;
     dim3 block(BKR_LINK_TILE, G);
     unsigned grid = (unsigned)std::min(ntiles, BKR_NUM_SMS * MINB);
+    static bool attr_done = false; // one flag per instantiation
+    if (!attr_done) {
+        BKR_CUDA(ctx, cudaFuncSetAttribute(dslash_kernel<Real, T, G, true, MINB, DD, RG>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+        BKR_CUDA(ctx, cudaFuncSetAttribute(dslash_kernel<Real, T, G, false, MINB, DD, RG>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
+        attr_done = true;
+    }
     if (N == T * G)
-        dslash_kernel<Real, T, G, true, MINB, DD><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
-                                                                               (Cx *)out, (const Cx *)xp, (Real)a, parity, done, opts);
+        dslash_kernel<Real, T, G, true, MINB, DD, RG><<<grid, block, SMEM, ctx->stream>>>(
+            ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in, (Cx *)out, (const Cx *)xp, (Real)a, parity, done, opts);
     else
-        dslash_kernel<Real, T, G, false, MINB, DD><<<grid, block, 0, ctx->stream>>>(ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in,
-                                                                                (Cx *)out, (const Cx *)xp, (Real)a, parity, done, opts);
+        dslash_kernel<Real, T, G, false, MINB, DD, RG><<<grid, block, SMEM, ctx->stream>>>(
+            ctx->g, N, ntiles, wt, ctx->tile_order, (const Cx *)in, (Cx *)out, (const Cx *)xp, (Real)a, parity, done, opts);
     return bkr_check_launch(ctx);
 }
 
@@ -330,18 +297,23 @@ template <typename Real>
 static int launch_n(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
 #define GO(T_, G_, M_) return launch_tg<Real, T_, G_, M_>(ctx, parity, N, in, out, xp, a, done)
-    static const char *cfg = getenv("BKR_DSLASH_CFG"); // tuning hook: "T,G,MINB,D"
+#ifdef BKR_TUNING
+    static const char *cfg = getenv("BKR_DSLASH_CFG"); // tuning hook (build with -DBKR_TUNING): "T,G,MINB,D,RG"
     if (cfg) {
-        int t = 0, gg = 0, mb = 0, dd = 0;
-        sscanf(cfg, "%d,%d,%d,%d", &t, &gg, &mb, &dd);
+        int t = 0, gg = 0, mb = 0, dd = 0, rg = 0;
+        sscanf(cfg, "%d,%d,%d,%d,%d", &t, &gg, &mb, &dd, &rg);
         if (N <= t * gg) {
-#define TRY(T_, G_, M_, D_) if (t == T_ && gg == G_ && mb == M_ && dd == D_) return launch_tg<Real, T_, G_, M_, D_>(ctx, parity, N, in, out, xp, a, done)
-            TRY(8, 2, 3, 6); TRY(8, 2, 3, 4); TRY(8, 2, 2, 12); TRY(8, 2, 2, 8); TRY(8, 2, 2, 24); TRY(4, 4, 2, 6); TRY(4, 4, 2, 4); TRY(4, 4, 2, 12);
-            TRY(6, 3, 2, 9); TRY(6, 3, 2, 6); TRY(8, 1, 4, 12); TRY(8, 1, 4, 8); TRY(8, 1, 6, 6); TRY(4, 2, 4, 6); TRY(4, 2, 4, 4); TRY(4, 2, 4, 12); TRY(4, 2, 3, 12);
-            TRY(8, 4, 1, 12); TRY(8, 4, 1, 24); TRY(8, 3, 1, 12); TRY(4, 8, 1, 6); TRY(4, 6, 1, 6); TRY(4, 6, 1, 12); TRY(4, 8, 1, 12);
+#define TRY(T_, G_, M_, D_, R_) if (t == T_ && gg == G_ && mb == M_ && dd == D_ && rg == R_) return launch_tg<Real, T_, G_, M_, D_, R_>(ctx, parity, N, in, out, xp, a, done)
+            TRY(8, 2, 2, 12, 2); TRY(8, 2, 2, 12, 4); TRY(8, 2, 2, 12, 8); TRY(8, 2, 3, 6, 4); TRY(8, 2, 3, 6, 8); TRY(8, 2, 2, 8, 8);
+            TRY(4, 4, 2, 12, 8); TRY(4, 4, 2, 6, 8); TRY(4, 4, 1, 24, 16); TRY(4, 4, 2, 12, 4); TRY(4, 4, 1, 12, 16);
+            TRY(8, 1, 4, 12, 4); TRY(8, 1, 3, 12, 8); TRY(8, 1, 2, 12, 16); TRY(4, 2, 4, 12, 4); TRY(4, 2, 3, 12, 8); TRY(4, 2, 2, 24, 16);
+            TRY(8, 4, 1, 12, 16); TRY(8, 4, 1, 12, 8); TRY(4, 8, 1, 12, 16); TRY(4, 8, 1, 6, 16); TRY(8, 3, 1, 12, 16); TRY(4, 6, 1, 12, 16);
 #undef TRY
+            fprintf(stderr, "BKR_DSLASH_CFG %s: not compiled in\n", cfg);
+            return BKR_EINVAL;
         }
     }
+#endif
     // Register budget decides the shape (ptxas -v: the fp64 T = 8 thread needs ~190 registers for 48 accumulators, the
     // 12-deep load ring and the link column; under a 168-register cap it spills ~0.5 KB per thread, and ncu showed the
     // spill traffic, not the stencil, filling the LSU).  fp64: at most 2 CTAs of 128 threads (or 4 of 64) per SM.

@@ -1,0 +1,509 @@
+// Multi-BLAS on native blocks v[j][k] (N vectors of L = 3 Vh complex, row index k contiguous):
+//   reduction multi-BLAS  K = X^dag Y          PAPER.md:272-299 (eq. 4)
+//   streaming multi-BLAS  Z = C + W a          PAPER.md:245-270 (eq. 3; Alg. 1 l.8, l.10, l.11, Alg. 2 l.4)
+// Both stream every vector element once, so memory traffic is linear in N.
+//
+// Design.  These kernels are HBM streams with a small dense contraction attached, and the
+// first version (one warp = 16 rows, loads -> DMMA -> loads -> stores in program order) was latency bound: ncu showed
+// 48 of 56 cycles per issued instruction on the long scoreboard and 42 % of DRAM bandwidth, because a warp had at most
+// 4 KB in flight.  Here the loads are taken off the warps altogether:
+//  * persistent CTAs (one per SM) of one producer warp and CW consumer warps;
+//  * the producer streams row tiles -- R rows of every vector of the block(s), one contiguous R x 16-byte chunk per
+//    vector -- into a shared-memory ring with 1-D TMA bulk copies (cp.async.bulk + mbarrier complete_tx, evict_first),
+//    so ~150 KB per SM are in flight whatever the register budget;
+//  * consumers read DMMA fragments from the ring with conflict-free 16-byte shared loads (the chunk stride is padded
+//    so that the 8 lanes of a quarter warp hit 8 different 16-byte bank groups) and never wait on global memory.
+// Arithmetic: both are tall-skinny complex GEMMs (inner or outer dimension N <= 32).  On B200 the FP64 tensor path
+// (DMMA m8n8k4) runs at the same peak as DFMA (measured 36.8 vs 36.7 TFLOP/s), so it raises no ceiling; it is used
+// because one DMMA replaces 8 DFMAs per lane and needs 2 operand registers for 8 FMAs.  A complex product is 4 real
+// DMMAs.  All accumulation is fp64 whatever the storage precision.  Reductions finish in a fixed order (no
+// floating-point atomics): results are bit-reproducible.
+#include "common.cuh"
+#include "tma.cuh"
+
+#include <stdlib.h>
+#include <string.h>
+
+static const int MB_SMEM_BUDGET = 216 * 1024; // of the 227 KB a CTA may opt in to
+static const int MB_MAX_STAGES = 8;
+
+__device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+        : "+d"(c[0]), "+d"(c[1])
+        : "d"(a), "d"(b));
+}
+
+// mbarrier wait that is also a compiler barrier for memory: the plain shared-memory reads of a stage must not move
+// above it
+__device__ __forceinline__ void mbar_wait_acq(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_addr(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void mbar_arrive_rel(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+
+template <typename Cx> __device__ __forceinline__ double2 sm_cx(const unsigned char *p)
+{
+    const Cx v = *reinterpret_cast<const Cx *>(p);
+    return make_double2((double)v.x, (double)v.y);
+}
+template <typename Cx> __device__ __forceinline__ void st_cx(Cx *p, double re, double im);
+template <> __device__ __forceinline__ void st_cx<double2>(double2 *p, double re, double im)
+{
+    __stcs(p, make_double2(re, im));
+}
+template <> __device__ __forceinline__ void st_cx<float2>(float2 *p, double re, double im)
+{
+    __stcs(p, make_float2((float)re, (float)im));
+}
+
+// Ring geometry shared by host and device.  A stage holds `nchunk_a` chunks of stride rs_a and `nchunk_b` chunks of
+// stride rs_b (bytes); a chunk is R consecutive rows of one vector.
+struct RingPlan {
+    int R, nstg;
+    uint32_t rs_a, rs_b, off_b, stage_bytes, off_ring; // off_ring: start of the ring in dynamic shared memory
+    size_t smem;
+};
+
+// pad: the residue (mod 128 bytes) the chunk stride must have so that fragment loads are conflict-free
+// Policy (measured, 32^4): a stage costs ~600 cycles of fixed overhead plus ~40 per bulk copy,
+// so R is the largest power of two that still leaves `min_stages` stages in the ring (3 for the reductions, 4 for the
+// updates, whose consumers also write) and gives every SM at least two row tiles.
+static RingPlan plan_ring(size_t L, size_t fixed, int min_stages, int nchunk_a, int esize_a, int pad_a, int nchunk_b,
+                          int esize_b, int pad_b)
+{
+    RingPlan best;
+    memset(&best, 0, sizeof(best));
+    fixed = (fixed + 127) / 128 * 128;
+    static const char *renv = getenv("BKR_MB_R"); // tuning hook: force the rows per stage
+    const int rforce = renv ? atoi(renv) : 0;
+    for (int R = 1024; R >= 64; R /= 2) {
+        RingPlan p;
+        p.R = R;
+        p.rs_a = (uint32_t)(R * esize_a + pad_a);
+        p.rs_b = (uint32_t)(R * esize_b + pad_b);
+        p.off_b = ((uint32_t)nchunk_a * p.rs_a + 127) / 128 * 128;
+        p.stage_bytes = (p.off_b + (uint32_t)nchunk_b * p.rs_b + 127) / 128 * 128;
+        p.off_ring = (uint32_t)fixed;
+        int n = (int)((MB_SMEM_BUDGET - fixed) / p.stage_bytes);
+        if (n > MB_MAX_STAGES) n = MB_MAX_STAGES;
+        p.nstg = n;
+        p.smem = fixed + (size_t)n * p.stage_bytes;
+        bool ok = n >= min_stages && (L + R - 1) / R >= (size_t)2 * BKR_NUM_SMS;
+        if (rforce) ok = R == rforce && n >= 2;
+        if (ok || R == 64) {
+            if (n < 2) p.nstg = 0; // does not fit at all (cannot happen for N <= 32)
+            best = p;
+            break;
+        }
+    }
+    return best;
+}
+
+// ------------------------------------------------------------------------------------------ streaming update
+// Z = C + W a  as  D(8 rows x 8 j) += A(8 rows x 4 i) B(4 i x 8 j) with DMMA m8n8k4:
+//   A[m][q] = W[4 is + q][row m]      lane = 4 m + q reads one complex (Re and Im) from the ring,
+//   B[q][n] = a[4 is + q][8 tj + n]   in fragment order (registers for N <= 16, shared memory above),
+//   Re Z += Wr ar - Wi ai      Im Z += Wr ai + Wi ar.
+// The accumulator fragment of lane (m, q) holds columns j = 8 tj + 2 q + r, r = 0, 1 of row m: C is read from the ring
+// and Z written to global memory in that layout (8 consecutive rows of 4 vectors per instruction: full 128-byte
+// segments).  Chunk strides: W = 32 (mod 128) bytes, C = 16 (mod 128): both fragment patterns are conflict-free.
+// Z may alias C (the tile of C is in shared memory before the rows of Z are written); Z must not alias W.
+template <typename RealZ, typename RealW, int NTJ, int NIS, bool HASC, int CW>
+__global__ void __launch_bounds__((CW + 1) * 32, 1)
+update_tma_kernel(size_t L, int N, RingPlan rp, const double2 *__restrict__ a, const typename CxT<RealZ>::type *C,
+                  const typename CxT<RealW>::type *__restrict__ W, typename CxT<RealZ>::type *Z, const int *done)
+{
+    typedef typename CxT<RealZ>::type CxZ;
+    typedef typename CxT<RealW>::type CxW;
+    constexpr bool BREG = NIS * NTJ <= 8; // coefficient fragments in registers
+    constexpr int NF = NIS * NTJ * 32;
+    extern __shared__ __align__(128) unsigned char dsm[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(dsm);
+    uint64_t *empty = full + MB_MAX_STAGES;
+    double *bre = reinterpret_cast<double *>(dsm + 128), *bim = bre + NF;
+    unsigned char *ring = dsm + rp.off_ring;
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < rp.nstg; s++) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], CW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int idx = threadIdx.x; idx < NF; idx += blockDim.x) {
+        const int ln = idx & 31, f = idx >> 5;
+        const int is = f / NTJ, tj = f % NTJ;
+        const int i = 4 * is + (ln & 3), j = 8 * tj + (ln >> 2);
+        const double2 v = (i < N && j < N) ? a[i * N + j] : make_double2(0.0, 0.0);
+        bre[idx] = v.x;
+        bim[idx] = v.y;
+    }
+    __syncthreads();
+
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const int my = (int)((ntiles > blockIdx.x) ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0);
+
+    if (warp == CW) { // ---------------- producer
+        const uint64_t pol = policy_evict_first();
+        for (int it = 0; it < my; it++) {
+            const int s = it % rp.nstg;
+            if (it >= rp.nstg) mbar_wait(&empty[s], ((it / rp.nstg) - 1) & 1);
+            const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
+            const uint32_t rows = (uint32_t)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
+            unsigned char *st = ring + (size_t)s * rp.stage_bytes;
+            if (lane == 0)
+                mbar_expect_tx(&full[s], (uint32_t)N * rows * (uint32_t)(sizeof(CxW) + (HASC ? sizeof(CxZ) : 0)));
+            __syncwarp();
+            if (lane < N) {
+                tma_load_1d_hint(st + (size_t)lane * rp.rs_a, W + (size_t)lane * L + r0, rows * (uint32_t)sizeof(CxW), &full[s], pol);
+                if (HASC)
+                    tma_load_1d_hint(st + rp.off_b + (size_t)lane * rp.rs_b, C + (size_t)lane * L + r0,
+                                     rows * (uint32_t)sizeof(CxZ), &full[s], pol);
+            }
+        }
+        return;
+    }
+
+    // ---------------- consumers
+    const int m = lane >> 2, q = lane & 3;
+    double ar[BREG ? NIS * NTJ : 1], ai[BREG ? NIS * NTJ : 1];
+    if (BREG) {
+#pragma unroll
+        for (int f = 0; f < NIS * NTJ; f++) {
+            ar[f] = bre[f * 32 + lane];
+            ai[f] = bim[f * 32 + lane];
+        }
+    }
+    for (int it = 0; it < my; it++) {
+        const int s = it % rp.nstg;
+        const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
+        const int rows = (int)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
+        const unsigned char *stW = ring + (size_t)s * rp.stage_bytes;
+        const unsigned char *stC = stW + rp.off_b;
+        mbar_wait_acq(&full[s], (it / rp.nstg) & 1);
+        for (int u = warp; u < rows / 8; u += CW) {
+            const int row = 8 * u + m;
+            double2 wf[NIS];
+#pragma unroll
+            for (int is = 0; is < NIS; is++) {
+                const int i = 4 * is + q;
+                wf[is] = i < N ? sm_cx<CxW>(stW + (size_t)i * rp.rs_a + (size_t)row * sizeof(CxW)) : make_double2(0.0, 0.0);
+            }
+            double zre[NTJ][2], zim[NTJ][2];
+#pragma unroll
+            for (int tj = 0; tj < NTJ; tj++) zre[tj][0] = zre[tj][1] = zim[tj][0] = zim[tj][1] = 0.0;
+#pragma unroll
+            for (int is = 0; is < NIS; is++) {
+#pragma unroll
+                for (int tj = 0; tj < NTJ; tj++) {
+                    const int f = is * NTJ + tj;
+                    const double br = BREG ? ar[f] : bre[f * 32 + lane], bi = BREG ? ai[f] : bim[f * 32 + lane];
+                    dmma(zre[tj], wf[is].x, br);
+                    dmma(zre[tj], wf[is].y, -bi);
+                    dmma(zim[tj], wf[is].x, bi);
+                    dmma(zim[tj], wf[is].y, br);
+                }
+            }
+#pragma unroll
+            for (int tj = 0; tj < NTJ; tj++) {
+#pragma unroll
+                for (int r = 0; r < 2; r++) {
+                    const int j = 8 * tj + 2 * q + r;
+                    if (j < N) {
+                        double re = zre[tj][r], im = zim[tj][r];
+                        if (HASC) {
+                            const double2 c = sm_cx<CxZ>(stC + (size_t)j * rp.rs_b + (size_t)row * sizeof(CxZ));
+                            re += c.x;
+                            im += c.y;
+                        }
+                        st_cx<CxZ>(Z + (size_t)j * L + r0 + row, re, im);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive_rel(&empty[s]);
+    }
+}
+
+template <typename RealZ, typename RealW, int NTJ, int NIS>
+static int update_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done)
+{
+    typedef typename CxT<RealZ>::type CxZ;
+    typedef typename CxT<RealW>::type CxW;
+    constexpr int CW = 8;
+    const size_t fixed = 128 + (size_t)2 * NIS * NTJ * 32 * sizeof(double);
+    const RingPlan rp = plan_ring(L, fixed, 4, N, (int)sizeof(CxW), 32, C ? N : 0, (int)sizeof(CxZ), 16);
+    if (rp.nstg < 2) return BKR_EINVAL;
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
+    static bool attr_done = false; // one flag per instantiation
+    if (!attr_done) {
+        BKR_CUDA(ctx, cudaFuncSetAttribute(update_tma_kernel<RealZ, RealW, NTJ, NIS, true, CW>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));
+        BKR_CUDA(ctx, cudaFuncSetAttribute(update_tma_kernel<RealZ, RealW, NTJ, NIS, false, CW>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));
+        attr_done = true;
+    }
+    if (C)
+        update_tma_kernel<RealZ, RealW, NTJ, NIS, true, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
+            L, N, rp, a, (const CxZ *)C, (const CxW *)W, (CxZ *)Z, done);
+    else
+        update_tma_kernel<RealZ, RealW, NTJ, NIS, false, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
+            L, N, rp, a, nullptr, (const CxW *)W, (CxZ *)Z, done);
+    return bkr_check_launch(ctx);
+}
+
+template <typename RealZ, typename RealW>
+static int launch_update_t(bkr_ctx *ctx, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done)
+{
+    const size_t L = (size_t)ctx->g.Vh * 3;
+    const int NIS = (N + 3) / 4;
+#define UPD_GO(NTJ_, NIS_) return update_go<RealZ, RealW, NTJ_, NIS_>(ctx, L, N, a, C, W, Z, done)
+    switch (NIS) {
+    case 1: UPD_GO(1, 1);
+    case 2: UPD_GO(1, 2);
+    case 3: UPD_GO(2, 3);
+    case 4: UPD_GO(2, 4);
+    case 5: UPD_GO(3, 5);
+    case 6: UPD_GO(3, 6);
+    case 7: UPD_GO(4, 7);
+    default: UPD_GO(4, 8);
+    }
+#undef UPD_GO
+}
+
+int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C, const void *W, void *Z,
+                        const int *done)
+{
+    if (precZ == BKR_F64 && precW == BKR_F64) return launch_update_t<double, double>(ctx, N, a, C, W, Z, done);
+    if (precZ == BKR_F64 && precW == BKR_F32) return launch_update_t<double, float>(ctx, N, a, C, W, Z, done);
+    if (precZ == BKR_F32 && precW == BKR_F32) return launch_update_t<float, float>(ctx, N, a, C, W, Z, done);
+    // fp32 <- fp64: only Qhat = R C^-1 of the reliable update (Alg. 3 l.5), computed in fp64, rounded on store
+    return launch_update_t<float, double>(ctx, N, a, C, W, Z, done);
+}
+
+// ------------------------------------------------------------------------------------------ Gram, stage 1
+// G = X^dag Y on 8 x 8 tiles of the N x N output, DMMA m8n8k4 over 4 rows at a time:
+//   A[m][q] = X[8 ti + m][k + q] (8 x 4),  B[q][n] = Y[8 tj + n][k + q] (4 x 8), lane = 4 m + q reads one complex
+//   of X (and of Y unless X == Y) from the ring with one 16-byte shared load, and
+//   Re G += Xr Yr + Xi Yi     Im G += Xr Yi - Xi Yr      (four accumulators per tile pair, combined at the end).
+// HERM: only pairs ti <= tj.  Otherwise blockIdx.y picks TIB i-tiles, all j-tiles.
+// Chunk stride = 64 (mod 128) bytes for fp64 and 32 (mod 128) for fp32: conflict-free fragment loads.  Chunk slots of
+// vectors >= N (padding of the last 8 x 8 tile) are never written by TMA; they are zeroed once, so no load in the loop
+// is predicated.  Deterministic: fixed tile -> CTA -> warp assignment, fixed-order warp reduction through shared
+// memory, one partial per CTA, fixed-order second stage.
+template <typename Real, int NT, bool HERM, bool ALIAS, int TIB, int CW>
+__global__ void __launch_bounds__((CW + 1) * 32, 1)
+gram_tma_kernel(size_t L, int N, RingPlan rp, const typename CxT<Real>::type *__restrict__ X,
+                const typename CxT<Real>::type *__restrict__ Y, double2 *__restrict__ partials, const int *done)
+{
+    typedef typename CxT<Real>::type Cx;
+    constexpr int NXT = HERM ? NT : TIB;                    // i-tiles this CTA touches
+    constexpr int NP = HERM ? NT * (NT + 1) / 2 : TIB * NT; // tile pairs this CTA accumulates
+    extern __shared__ __align__(128) unsigned char dsm[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(dsm);
+    uint64_t *empty = full + MB_MAX_STAGES;
+    double2 *red = reinterpret_cast<double2 *>(dsm + 128); // [N * N]
+    unsigned char *ring = dsm + rp.off_ring;
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int ti0 = HERM ? 0 : blockIdx.y * TIB;
+    const int i0 = 8 * ti0;                                  // first X vector of this CTA
+    const int nxv = min(N - i0, 8 * NXT);                    // X vectors this CTA loads
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < rp.nstg; s++) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], CW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // zero the whole ring once (padding chunk slots stay zero; TMA overwrites the rest)
+    {
+        uint4 *z = reinterpret_cast<uint4 *>(ring);
+        const size_t n16 = (size_t)rp.nstg * rp.stage_bytes / 16;
+        for (size_t o = threadIdx.x; o < n16; o += blockDim.x) z[o] = make_uint4(0, 0, 0, 0);
+    }
+    for (int o = threadIdx.x; o < N * N; o += blockDim.x) red[o] = make_double2(0.0, 0.0);
+    // generic-proxy writes (the zeroing) before async-proxy writes (TMA) to the same shared memory
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const int my = (int)((ntiles > blockIdx.x) ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0);
+
+    if (warp == CW) { // ---------------- producer
+        const uint64_t pol = policy_evict_first();
+        for (int it = 0; it < my; it++) {
+            const int s = it % rp.nstg;
+            if (it >= rp.nstg) mbar_wait(&empty[s], ((it / rp.nstg) - 1) & 1);
+            const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
+            const uint32_t rows = (uint32_t)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
+            unsigned char *st = ring + (size_t)s * rp.stage_bytes;
+            if (lane == 0) mbar_expect_tx(&full[s], (uint32_t)(nxv + (ALIAS ? 0 : N)) * rows * (uint32_t)sizeof(Cx));
+            __syncwarp();
+            if (lane < nxv)
+                tma_load_1d_hint(st + (size_t)lane * rp.rs_a, X + (size_t)(i0 + lane) * L + r0, rows * (uint32_t)sizeof(Cx), &full[s], pol);
+            if (!ALIAS && lane < N)
+                tma_load_1d_hint(st + rp.off_b + (size_t)lane * rp.rs_b, Y + (size_t)lane * L + r0, rows * (uint32_t)sizeof(Cx), &full[s], pol);
+        }
+        return;
+    }
+
+    // ---------------- consumers
+    const int m = lane >> 2, q = lane & 3;
+    double acc[NP][4][2]; // Xr Yr, Xr Yi, Xi Yr, Xi Yi: four independent DMMA chains per tile pair
+#pragma unroll
+    for (int p = 0; p < NP; p++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) acc[p][c][0] = acc[p][c][1] = 0.0;
+
+    for (int it = 0; it < my; it++) {
+        const int s = it % rp.nstg;
+        const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
+        const int rows = (int)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
+        const unsigned char *stX = ring + (size_t)s * rp.stage_bytes;
+        const unsigned char *stY = ALIAS ? stX : stX + rp.off_b;
+        const uint32_t rsy = ALIAS ? rp.rs_a : rp.rs_b;
+        mbar_wait_acq(&full[s], (it / rp.nstg) & 1);
+        // a k-step = 4 rows; two k-steps per iteration (fragments of both loaded before the first DMMA) so that the
+        // shared-memory latency of one hides behind the tensor work of the other even with one warp per scheduler
+        const int nks = rows / 4;
+        for (int ks = warp; ks < nks; ks += 2 * CW) {
+            const bool two = ks + CW < nks;
+            double2 xf[2][NXT], yf[2][ALIAS ? 1 : NT];
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const size_t ro = (size_t)(4 * (ks + (h && two ? CW : 0)) + q) * sizeof(Cx);
+#pragma unroll
+                for (int t = 0; t < NXT; t++) xf[h][t] = sm_cx<Cx>(stX + (size_t)(8 * t + m) * rp.rs_a + ro);
+                if (!ALIAS) {
+#pragma unroll
+                    for (int t = 0; t < NT; t++) yf[h][t] = sm_cx<Cx>(stY + (size_t)(8 * t + m) * rsy + ro);
+                }
+            }
+            if (!two) { // odd tail: the second k-step contributes nothing
+#pragma unroll
+                for (int t = 0; t < NXT; t++) xf[1][t] = make_double2(0.0, 0.0);
+            }
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                int p = 0;
+#pragma unroll
+                for (int ti = 0; ti < NXT; ti++) {
+#pragma unroll
+                    for (int tj = HERM ? ti : 0; tj < NT; tj++, p++) {
+                        const double2 a = xf[h][ti];
+                        const double2 b = ALIAS ? xf[h][tj] : yf[h][tj];
+                        dmma(acc[p][0], a.x, b.x);
+                        dmma(acc[p][1], a.x, b.y);
+                        dmma(acc[p][2], a.y, b.x);
+                        dmma(acc[p][3], a.y, b.y);
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive_rel(&empty[s]);
+    }
+
+    // fixed-order reduction over the consumer warps of the CTA, then one partial per CTA.  Named barrier 1 over the
+    // consumer warps only (the producer warp has returned).
+    for (int w = 0; w < CW; w++) {
+        if (warp == w) {
+            int p = 0;
+#pragma unroll
+            for (int ti = 0; ti < NXT; ti++) {
+#pragma unroll
+                for (int tj = HERM ? ti : 0; tj < NT; tj++, p++) {
+#pragma unroll
+                    for (int r = 0; r < 2; r++) {
+                        const int i = 8 * (ti0 + ti) + m, j = 8 * tj + 2 * q + r;
+                        if (i < N && j < N) {
+                            double2 v = red[i * N + j];
+                            v.x += acc[p][0][r] + acc[p][3][r];
+                            v.y += acc[p][1][r] - acc[p][2][r];
+                            red[i * N + j] = v;
+                        }
+                    }
+                }
+            }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(CW * 32) : "memory");
+    }
+    const int row0 = 8 * ti0, row1 = HERM ? N : min(N, 8 * (ti0 + TIB));
+    for (int o = row0 * N + threadIdx.x; o < row1 * N; o += CW * 32)
+        partials[(size_t)blockIdx.x * N * N + o] = red[o];
+}
+
+static const int GRAM_MAX_GRID = BKR_NUM_SMS;
+
+template <typename Real, int NT>
+static int gram_go(bkr_ctx *ctx, size_t L, int N, const void *X, const void *Y, int hermitian, int *num_partials, const int *done)
+{
+    typedef typename CxT<Real>::type Cx;
+    constexpr int TIB = NT > 2 ? 2 : NT;
+    constexpr int CW = NT > 2 ? 4 : 8; // above two tiles the accumulators need the 255-register budget of 160 threads
+    const Cx *x = (const Cx *)X, *y = (const Cx *)Y;
+    const bool alias = hermitian && X == Y;
+    const int pad = sizeof(Real) == 8 ? 64 : 32;
+    const size_t fixed = 128 + (size_t)N * N * sizeof(double2);
+    const int nxs = hermitian ? 8 * NT : 8 * TIB; // X chunk slots (vectors >= N: zero padding)
+    const RingPlan rp = plan_ring(L, fixed, 3, nxs, (int)sizeof(Cx), pad, alias ? 0 : 8 * NT, (int)sizeof(Cx), pad);
+    if (rp.nstg < 2) return BKR_EINVAL;
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const unsigned gx = (unsigned)(ntiles < (size_t)GRAM_MAX_GRID ? ntiles : (size_t)GRAM_MAX_GRID);
+#define GRAM_LAUNCH(H_, A_, TIB_, GRID_)                                                                               \
+    do {                                                                                                               \
+        static bool attr_done = false;                                                                                 \
+        if (!attr_done) {                                                                                              \
+            BKR_CUDA(ctx, cudaFuncSetAttribute(gram_tma_kernel<Real, NT, H_, A_, TIB_, CW>,                            \
+                                               cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));          \
+            attr_done = true;                                                                                          \
+        }                                                                                                              \
+        gram_tma_kernel<Real, NT, H_, A_, TIB_, CW><<<GRID_, (CW + 1) * 32, rp.smem, ctx->stream>>>(L, N, rp, x, y,     \
+                                                                                                   ctx->partials, done); \
+    } while (0)
+    if (hermitian) {
+        if (alias) GRAM_LAUNCH(true, true, NT, gx);
+        else GRAM_LAUNCH(true, false, NT, gx);
+    } else {
+        dim3 g2(gx, (NT + TIB - 1) / TIB);
+        GRAM_LAUNCH(false, false, TIB, g2);
+    }
+#undef GRAM_LAUNCH
+    *num_partials = (int)gx;
+    return bkr_check_launch(ctx);
+}
+
+int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, int *num_partials,
+                         const int *done)
+{
+    const size_t L = (size_t)ctx->g.Vh * 3;
+    BKR_TRY(ensure_partials(ctx, (size_t)2 * BKR_NUM_SMS * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
+    const int NT = (N + 7) / 8;
+#define GRAM_NT(Real)                                                                    \
+    switch (NT) {                                                                        \
+    case 1: return gram_go<Real, 1>(ctx, L, N, X, Y, hermitian, num_partials, done);     \
+    case 2: return gram_go<Real, 2>(ctx, L, N, X, Y, hermitian, num_partials, done);     \
+    case 3: return gram_go<Real, 3>(ctx, L, N, X, Y, hermitian, num_partials, done);     \
+    default: return gram_go<Real, 4>(ctx, L, N, X, Y, hermitian, num_partials, done);    \
+    }
+    if (prec == BKR_F64) {
+        GRAM_NT(double)
+    }
+    GRAM_NT(float)
+#undef GRAM_NT
+}
