@@ -285,6 +285,24 @@ def run_reference(args):
     return 0
 
 
+# ---------------------------------------------------------------- multi-GPU aggregation ("replicas only")
+
+def max_over_ranks(dist, value, device):
+    """MAX all-reduce of a host scalar (the timing of the slowest replica); identity without a process group."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def replicas_value(world, bytes_per_step_per_rank, ms_step_max):
+    """whole-job throughput of `world` independent replicas (no data-path collective): every
+    rank moves the same algorithmic bytes per step; the job takes as long as its slowest rank."""
+    return world * bytes_per_step_per_rank / ms_step_max * 1e-6
+
+
 # ---------------------------------------------------------------- the CUDA path
 
 def run_bkr(args):
@@ -333,14 +351,10 @@ def run_bkr(args):
     torch.cuda.synchronize()
     if dist:
         dist.barrier()
-    ms_total = e0.elapsed_time(e1)
-    if dist:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(dist, e0.elapsed_time(e1), dev)
     ms_step = ms_total / args.steps
     by_iter = bytes_iteration(dims, N, w)
-    value = world * by_iter / ms_step * 1e-6
+    value = replicas_value(world, by_iter, ms_step)
 
     # ---- the dominant kernel alone (multi-rhs Dslash), and the multi-BLAS kernels, at this N
     kern = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=max(50, args.steps), warmup=3, hbm=hbm)
@@ -361,10 +375,7 @@ def run_bkr(args):
         rr, st = ctx.solve_block_host(mass, Bh, Xh, tol=1e-10, maxiter=args.steps, inner_prec=prec)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if dist:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dist, dt, dev)
         k = max(1, st["iters"])
         e2e = {"value": world * k * by_iter / dt * 1e-9, "unit": "GB/s",
                "h2d_bytes_per_step": 2 * Bh.numel() * 16 / k, "d2h_bytes_per_step": Xh.numel() * 16 / k,

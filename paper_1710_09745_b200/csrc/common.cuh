@@ -9,6 +9,19 @@
 #define BKR_NUM_SMS 148 /* B200: 2 dies x 74 SMs; grids are sized in multiples of this */
 #define BKR_LINK_TILE 64 /* sites per link tile: one TMA bulk copy per (tile, hop) = 9 * 64 complex */
 
+// Order of the 16 hops in the gather-form link stream and in the stencil's hop loop:
+//   y-3, y-1, x+1, x-1, x+3, x-3, y+1, y+3, z-3, z-1, z+1, z+3, t-3, t-1, t+1, t+3.
+// For a tile of consecutive x-rows (y0 .. y0+3) consecutive hops then read overlapping sets of input rows
+// (y0-3..y0, y0-1..y0+2, y0..y0+3 four times, y0+1..y0+4, y0+3..y0+6), so every L1 reuse has distance one hop -- the
+// only distance at which the per-hop footprint of N x 48 bytes per site survives in L1 (ncu: with the order x, y+1, y-1,
+// y+3, y-3 the L1 hit rate was 24 % against 34 % possible).  Encoded as bit fields indexed by the hop number h.
+#define BKR_HOP_MU_BITS 0xffaa5005u /* 2 bits per hop: direction mu */
+#define BKR_HOP_LONG_BITS 0x99b1u /* 1 bit per hop: 1 = long link (three sites) */
+#define BKR_HOP_BACK_BITS 0x332bu /* 1 bit per hop: 1 = backward */
+#define BKR_HOP_MU(h) ((BKR_HOP_MU_BITS >> (2 * (h))) & 3u)
+#define BKR_HOP_LONG(h) ((BKR_HOP_LONG_BITS >> (h)) & 1u)
+#define BKR_HOP_BACK(h) ((BKR_HOP_BACK_BITS >> (h)) & 1u)
+
 struct Geom {
     int X[4];     // extents x,y,z,t (all even, >= 4)
     int V, Vh;    // sites, sites per parity (48^3 x 96 = 10.6 M fits an int)

@@ -107,13 +107,13 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
         // flight to cover L2/HBM latency at 12-16 warps per SM (measured: the compiler's own schedule kept ~2.4).
         const int st0 = k * 16;
         auto nbr = [&](int h) -> const Cx * {
-            const int mu = h >> 2, hop = (h & 2) ? 3 : 1;
+            const int mu = BKR_HOP_MU(h), hop = BKR_HOP_LONG(h) ? 3 : 1;
             const int cm = mu == 0 ? c[0] : mu == 1 ? c[1] : mu == 2 ? c[2] : c[3];
             // select chains, not g.X[mu]: an indexed constant load is a scoreboarded (variable-latency) load, and the
             // in-order warp waited for it at the top of every hop (ncu source page: 8 % of all warp time)
             const int Xm = mu == 0 ? g.X[0] : mu == 1 ? g.X[1] : mu == 2 ? g.X[2] : g.X[3];
             const int sm = mu == 0 ? 1 : mu == 1 ? g.X[0] : mu == 2 ? g.X[0] * g.X[1] : g.X[0] * g.X[1] * g.X[2];
-            int cn = (h & 1) ? cm - hop : cm + hop;
+            int cn = BKR_HOP_BACK(h) ? cm - hop : cm + hop;
             if (cn < 0) cn += Xm;
             if (cn >= Xm) cn -= Xm;
             return vin + ((s + (cn - cm) * sm) >> 1);

@@ -9,8 +9,9 @@
 //   native links  Wt[p][tile][h][el][lane] : gather form, tile-major (see pack_links_kernel below).
 #include "common.cuh"
 
-// Gather-form links.  For the output site x of parity p (even-odd index e) and hop h = ((mu*2 + type)*2 + dir)
-// (type 0 fat / 1 long, hop length 1 / 3; dir 0 forward / 1 backward) the stencil needs the matrix
+// Gather-form links.  For the output site x of parity p (even-odd index e) and hop h = 0..15 in the order of
+// common.cuh (BKR_HOP_*: direction mu, type 0 fat / 1 long = hop length 1 / 3, dir 0 forward / 1 backward) the
+// stencil needs the matrix
 //     W_h(x) = U_mu(x)                (forward)         W_h(x) = - U_mu(x - hop mu)^dagger   (backward)
 // so that (D in)(x) = sum_h W_h(x) in(nbr_h(x))  (eq. 2).  Storing W per output site makes the
 // whole link stream of a tile of BKR_LINK_TILE consecutive sites ONE contiguous chunk
@@ -29,7 +30,7 @@ __global__ void pack_links_kernel(Geom g, int ntiles, const double2 *__restrict_
     const size_t r = tid / 16;
     const int e = (int)(r % padded);
     const int parity = (int)(r / padded);
-    const int mu = h >> 2, type = (h >> 1) & 1, dir = h & 1;
+    const int mu = BKR_HOP_MU(h), type = BKR_HOP_LONG(h), dir = BKR_HOP_BACK(h);
     const size_t base = ((((size_t)parity * ntiles + e / BKR_LINK_TILE) * 16 + h) * 9) * BKR_LINK_TILE + e % BKR_LINK_TILE;
     double2 w[9];
     if (e < g.Vh) {
