@@ -47,6 +47,7 @@ int bkr_destroy(bkr_ctx *ctx)
     cudaFree(ctx->links64);
     cudaFree(ctx->links32);
     cudaFree(ctx->tile_order);
+    cudaFree(ctx->win_segs);
     cudaFree(ctx->tmp_odd[0]);
     cudaFree(ctx->tmp_odd[1]);
     cudaFree(ctx->partials);

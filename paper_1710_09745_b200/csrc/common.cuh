@@ -54,6 +54,9 @@ struct bkr_ctx {
     // tile processing order of the stencil (L2 blocking, dslash.cu): device table + the blocking it was built for
     int *tile_order;
     int tile_order_key;
+    // segment table of the window stencil (dslash_win.cu): (first tile, end tile, strip first, strip last)
+    int4 *win_segs;
+    int win_nseg, win_key;
     // scratch for apply_M (odd-parity temporary), grown on demand, per precision
     void *tmp_odd[2];
     size_t tmp_odd_bytes[2];
@@ -106,6 +109,10 @@ int launch_convert(bkr_ctx *ctx, size_t n_complex, int src_prec, const void *src
 // ---- dslash.cu :  out = D in   or (xpay) out = a * xp - D in
 int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp,
                   double a, const int *done);
+
+// ---- dslash_win.cu : same operation, shared-memory window version; returns 1 when not applicable
+int launch_dslash_win(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp,
+                      double a, const int *done);
 
 // ---- blas.cu
 // stage 1 of K = X^dag Y: per-CTA partial sums into ctx->partials; returns the number of partials.
