@@ -142,6 +142,12 @@ int bkr_solve_cg_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void
 int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void *B, int iters,
                          long long *launches);
 
+/* Which stencil kernel the most recent Dslash launch of this context used (bkr_dslash, bkr_apply_M or inside a solver):
+ * 0 = plain multi-rhs kernel (register tiling + link ring), 1 = shared-memory window kernel with
+ * cluster-multicast links (same operation; chosen per lattice/N/precision),
+ * -1 = none yet.  Diagnostic only. */
+int bkr_dslash_variant(const bkr_ctx *ctx);
+
 int bkr_last_cuda_error(const bkr_ctx *ctx);
 const char *bkr_strerror(int status);
 const char *bkr_version(void);

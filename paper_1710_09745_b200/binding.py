@@ -21,7 +21,7 @@ SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash",
     "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
-    "bkr_strerror", "bkr_version",
+    "bkr_strerror", "bkr_version", "bkr_dslash_variant",
 )
 
 
@@ -75,6 +75,7 @@ def lib():
             "bkr_last_cuda_error": (ci, [vp]),
             "bkr_strerror": (ctypes.c_char_p, [ci]),
             "bkr_version": (ctypes.c_char_p, []),
+            "bkr_dslash_variant": (ci, [vp]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name)
@@ -267,6 +268,10 @@ class Context:
         self._check(lib().bkr_bench_iterations(self._h, float(mass), N, int(prec), _dev_ptr(B, "B"), int(iters),
                                                ctypes.byref(n)), "bkr_bench_iterations")
         return int(n.value)
+
+    def dslash_variant(self):
+        """0 = plain stencil kernel, 1 = shared-memory window kernel, -1 = no Dslash launched yet (diagnostic)."""
+        return int(lib().bkr_dslash_variant(self._h))
 
 
 def version():

@@ -29,6 +29,7 @@ int bkr_create(bkr_ctx **out, const int dims[4], int device, void *cuda_stream)
     ctx->g.V = (int)V;
     ctx->g.Vh = (int)(V / 2);
     ctx->device = device;
+    ctx->dslash_variant = -1;
     ctx->stream = (cudaStream_t)cuda_stream;
     if (cudaMalloc((void **)&ctx->small, (size_t)4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)) != cudaSuccess) {
         free(ctx);
@@ -241,6 +242,8 @@ const char *bkr_strerror(int status)
     default: return "unknown status";
     }
 }
+
+int bkr_dslash_variant(const bkr_ctx *ctx) { return ctx ? ctx->dslash_variant : -1; }
 
 const char *bkr_version(void) { return "libbkr 0.1 (sm_100a)"; }
 

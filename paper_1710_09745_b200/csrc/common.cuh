@@ -57,6 +57,7 @@ struct bkr_ctx {
     // segment table of the window stencil (dslash_win.cu): (first tile, end tile, strip first, strip last)
     int4 *win_segs;
     int win_nseg, win_key;
+    int dslash_variant; // last stencil kernel used: 0 plain, 1 window, -1 none yet
     // scratch for apply_M (odd-parity temporary), grown on demand, per precision
     void *tmp_odd[2];
     size_t tmp_odd_bytes[2];

@@ -350,8 +350,12 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
     if (!(prec == BKR_F64 ? (void *)ctx->links64 : (void *)ctx->links32)) return BKR_ENOLINKS;
     {
         const int rc = launch_dslash_win(ctx, out_parity, N, prec, in, out, xp, a, done);
-        if (rc != 1) return rc;
+        if (rc != 1) {
+            ctx->dslash_variant = 1;
+            return rc;
+        }
     }
+    ctx->dslash_variant = 0;
     BKR_TRY(build_tile_order(ctx, N, prec));
     if (prec == BKR_F64) return launch_n<double>(ctx, out_parity, N, in, out, xp, a, done);
     return launch_n<float>(ctx, out_parity, N, in, out, xp, a, done);

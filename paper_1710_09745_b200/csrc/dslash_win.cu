@@ -36,7 +36,6 @@
 #include <vector>
 
 #define WIN_CHUNK 32 /* sites per window chunk */
-#define WIN_RL 4     /* link ring stages (divides 16) */
 
 struct WinParams {
     Geom g;
@@ -51,6 +50,7 @@ struct WinParams {
     int HcL;    // window reach below/above a tile, in chunks
     int WCH;    // window ring slots (chunks)
     int nzlog;  // log2 of the z/t stage ring depth
+    int rllog;  // log2 of the link ring depth (2 or 3)
     int opts;   // tuning bits (BKR_WIN_OPTS): 1 = L2 prefetch of the next tile's links, 2 = of its z/t stages (no gain measured)
     uint32_t off_win, off_zt, off_red, off_bar;
 };
@@ -142,7 +142,6 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
     constexpr uint32_t LSTAGE = 9 * 64 * sizeof(Cx);
     constexpr uint32_t WCHUNK = NC * 3 * WIN_CHUNK * sizeof(Cx);
     constexpr uint32_t ZSTAGE = NC * 3 * 64 * sizeof(Cx); // one z/t hop: [rhs][colour][64 sites]
-    constexpr int RL = WIN_RL;
     extern __shared__ __align__(1024) unsigned char dsm[];
     unsigned char *const lnk = dsm;
     unsigned char *const win = dsm + p.off_win;
@@ -153,7 +152,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                     *const zfull = bar + 48, *const zempty = bar + 56, *const redfull = bar + 64, *const redempty = bar + 65;
     if (p.done && *p.done) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int NZ = 1 << p.nzlog, WCH = p.WCH, HcL = p.HcL;
+    const int nzlog = p.nzlog, NZ = 1 << nzlog, rllog = p.rllog, RL = 1 << rllog, WCH = p.WCH, HcL = p.HcL;
     if (threadIdx.x == 0) {
         for (int s = 0; s < RL; s++) {
             mbar_init(&lfull[s], 1);
@@ -180,6 +179,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
     const int Xh = g.X[0] >> 1;
     const int Vh = g.Vh;
 
+    const bool dry = (p.opts & 4) != 0; // tuning probe: no producers, no barriers (results are garbage)
     if (warp >= 2 * NWS) {
         // ------------------------------------------------------------------ producers: one lane in each of 3 warps
         //   role 0: link stages of set A (even sequence numbers) and the window chunks
@@ -189,7 +189,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
         // stage is also requested into L2 one tile ahead (cp.async.bulk.prefetch.L2): the HBM latency is paid there,
         // the shared-memory rings only have to cover the L2 -> SM latency.
         const int role = warp - 2 * NWS;
-        if (lane == 0) {
+        if (lane == 0 && !dry) {
             const uint64_t pol = policy_evict_first();
             const Cx *wt = reinterpret_cast<const Cx *>(p.wt);
             const int XhY = Xh * g.X[1];
@@ -224,7 +224,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                     const int knext = k + 1 < sg.y ? k + 1 : (has_next ? sn.x : -1); // this CTA's next tile
                     if (role == 2) {
                         for (int j = 0; j < 8; j++) {
-                            const int zs = 8 * tc + j, slot = zs & (NZ - 1), use = zs >> p.nzlog;
+                            const int zs = 8 * tc + j, slot = zs & (NZ - 1), use = zs >> nzlog;
                             if (use > 0) mbar_wait(&zempty[slot], (use - 1) & 1);
                             mbar_expect_tx(&zfull[slot], ZSTAGE);
                             tma_load_3d(zt + (size_t)slot * ZSTAGE, &tm_zt, 2 * zt_src(k, 8 + j), 0, (int)rank * NC, &zfull[slot]);
@@ -250,7 +250,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                     if (role == 0 && k == sg.x) load_chunks(min(2 * k + 1 + HcL, seg_hi));
                     for (int j = 0; j < 8; j++) {
                         const int h = role ? 8 + j : j;
-                        const int ls = 16 * tc + 2 * j + role, slot = ls & (RL - 1), use = ls / RL;
+                        const int ls = 16 * tc + 2 * j + role, slot = ls & (RL - 1), use = ls >> rllog;
                         if (use > 0) mbar_wait(&lempty[slot], (use - 1) & 1);
                         mbar_expect_tx(&lfull[slot], LSTAGE);
                         const unsigned char *src = reinterpret_cast<const unsigned char *>(wt + ((size_t)k * 16 + h) * 9 * 64);
@@ -286,7 +286,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 const int whi = 2 * k + 1 + HcL;
                 while (waited <= whi) {
                     const int qq = q0 + waited - seg_lo;
-                    mbar_wait(&wfull[qq % WCH], (qq / WCH) & 1);
+                    if (!dry) mbar_wait(&wfull[qq % WCH], (qq / WCH) & 1);
                     waited++;
                 }
                 const int slot2k = (q0 + 2 * k - seg_lo) % WCH;
@@ -324,7 +324,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                     const Cx *wp = reinterpret_cast<const Cx *>(win + (size_t)sidx * WCHUNK) + j0 * 3 * WIN_CHUNK + (d & 31);
                     const int ls = 16 * tc + 2 * h, slot = ls & (RL - 1);
                     const Cx(*lk)[64] = reinterpret_cast<const Cx(*)[64]>(lnk + (size_t)slot * LSTAGE);
-                    mbar_wait(&lfull[slot], (ls / RL) & 1);
+                    if (!dry) mbar_wait(&lfull[slot], (ls >> rllog) & 1);
                     // the whole 3 x 3 matrix goes to registers and the slot back to the producer before the arithmetic:
                     // the ring then holds (almost) only data in flight
                     Cx u[3][3]; // u[b][a] = W_ab
@@ -333,7 +333,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
 #pragma unroll
                         for (int aa = 0; aa < 3; aa++) u[b][aa] = lds_cx(&lk[aa * 3 + b][sl]);
                     __syncwarp();
-                    if (lane == 0) {
+                    if (lane == 0 && !dry) {
                         if (C == 1) mbar_arrive(&lempty[slot]);
                         else
                             for (uint32_t r = 0; r < (uint32_t)C; r++) mbar_arrive_remote(&lempty[slot], r);
@@ -351,12 +351,12 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 {
                     const int new_rel = (k == sg.y - 1) ? seg_hi + 1 : 2 * (k + 1) - HcL;
                     __syncwarp();
-                    if (lane == 0)
+                    if (lane == 0 && !dry)
                         for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(q0 + cc - seg_lo) % WCH]);
                     released = max(released, new_rel);
                 }
                 // hand the partial sums to set B, which finishes the tile
-                if (tc > 0) mbar_wait_mem(redempty, (tc - 1) & 1);
+                if (tc > 0 && !dry) mbar_wait_mem(redempty, (tc - 1) & 1);
 #pragma unroll
                 for (int i = 0; i < T; i++)
 #pragma unroll
@@ -366,7 +366,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         o.y = acc[i][2 * cc + 1];
                         red[((j0 + i) * 3 + cc) * 64 + sl] = o;
                     }
-                mbar_arrive_mem(redfull);
+                if (!dry) mbar_arrive_mem(redfull);
             }
             q0 += seg_hi - seg_lo + 1;
         }
@@ -389,21 +389,21 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 for (int j = 0; j < 8; j++) {
                     const int ls = 16 * tc + 2 * j + 1, slot = ls & (RL - 1);
                     const Cx(*lk)[64] = reinterpret_cast<const Cx(*)[64]>(lnk + (size_t)slot * LSTAGE);
-                    mbar_wait(&lfull[slot], (ls / RL) & 1);
+                    if (!dry) mbar_wait(&lfull[slot], (ls >> rllog) & 1);
                     Cx u[3][3];
 #pragma unroll
                     for (int b = 0; b < 3; b++)
 #pragma unroll
                         for (int aa = 0; aa < 3; aa++) u[b][aa] = lds_cx(&lk[aa * 3 + b][sl]);
                     __syncwarp();
-                    if (lane == 0) {
+                    if (lane == 0 && !dry) {
                         if (C == 1) mbar_arrive(&lempty[slot]);
                         else
                             for (uint32_t r = 0; r < (uint32_t)C; r++) mbar_arrive_remote(&lempty[slot], r);
                     }
                     const int zs = 8 * tc + j, zslot = zs & (NZ - 1);
                     const Cx *zp = reinterpret_cast<const Cx *>(zt + (size_t)zslot * ZSTAGE) + j0 * 3 * 64 + sl;
-                    mbar_wait(&zfull[zslot], (zs >> p.nzlog) & 1);
+                    if (!dry) mbar_wait(&zfull[zslot], (zs >> nzlog) & 1);
 #pragma unroll
                     for (int b = 0; b < 3; b++) {
                         Cx v[T];
@@ -411,7 +411,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         for (int i = 0; i < T; i++) v[i] = lds_cx(zp + (i * 3 + b) * 64);
                         if (b == 2) {
                             __syncwarp();
-                            if (lane == 0) mbar_arrive(&zempty[zslot]);
+                            if (lane == 0 && !dry) mbar_arrive(&zempty[zslot]);
                         }
 #pragma unroll
                         for (int i = 0; i < T; i++) cfma3<Real, Cx>(acc[i], u[b], v[i]);
@@ -420,7 +420,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 const int e = k * 64 + sl;
                 Cx *vout = reinterpret_cast<Cx *>(p.out) + (size_t)jg * 3 * Vh + e;
                 const Cx *vxp = p.xp ? reinterpret_cast<const Cx *>(p.xp) + (size_t)jg * 3 * Vh + e : nullptr;
-                mbar_wait_mem(redfull, tc & 1);
+                if (!dry) mbar_wait_mem(redfull, tc & 1);
 #pragma unroll
                 for (int i = 0; i < T; i++)
 #pragma unroll
@@ -429,7 +429,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         acc[i][2 * cc] += rb.x;
                         acc[i][2 * cc + 1] += rb.y;
                     }
-                mbar_arrive_mem(redempty);
+                if (!dry) mbar_arrive_mem(redempty);
 #pragma unroll
                 for (int i = 0; i < T; i++) {
                     if (jg + i < p.N) {
@@ -528,7 +528,11 @@ static int build_segments(bkr_ctx *ctx, int N, int prec, int seglen)
     return BKR_OK;
 }
 
-static const size_t WIN_SMEM_MAX = 232448; // 227 KB opt-in limit per CTA
+static const size_t WIN_SMEM_MAX = 232448;
+// window slots beyond the 2 HcL + 2 chunks a tile reads: two, for the next tile's new chunks.  (Reusing the slots
+// below the tile, which are dead after the y-3, y-1 hops, saves 24 KB but makes the link producer wait for set A in
+// the middle of every tile: measured 0.72 -> 0.69 ms at N = 8 with the two spare slots.)
+static int HcLextra(int HcL) { (void)HcL; return 2; } // 227 KB opt-in limit per CTA
 
 // returns 1 if this instantiation cannot run the geometry (caller falls back), BKR_OK after a launch, else an error
 template <typename Real, int T, int G, int C>
@@ -542,18 +546,30 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     WinParams p;
     memset(&p, 0, sizeof(p));
     p.HcL = (3 * Xh + WIN_CHUNK - 1) / WIN_CHUNK;
-    p.WCH = 2 * p.HcL + 4;
+    p.WCH = 2 * p.HcL + 2 + HcLextra(p.HcL);
     if (p.WCH > 16) return 1;
-    const size_t lbytes = (size_t)WIN_RL * 9 * 64 * sizeof(Cx), wbytes = (size_t)p.WCH * NC * 3 * WIN_CHUNK * sizeof(Cx),
+    const size_t lstage = (size_t)9 * 64 * sizeof(Cx), wbytes = (size_t)p.WCH * NC * 3 * WIN_CHUNK * sizeof(Cx),
                  zstage = (size_t)NC * 3 * 64 * sizeof(Cx), rbytes = (size_t)NC * 3 * 64 * sizeof(Cx), bbytes = 66 * 8;
-    const char *zenv = getenv("BKR_WIN_NZLOG");
-    int nzlog = zenv ? atoi(zenv) : 1;
-    while (nzlog >= 0 && lbytes + wbytes + (zstage << nzlog) + rbytes + bbytes > WIN_SMEM_MAX) nzlog--;
-    if (nzlog < 0) return 1;
-    p.nzlog = nzlog;
+    // ring depths: as much data in flight as the 227 KB allow (the rings are what hides the ~1 us refill round trip);
+    // measured at 32^3 x 64, N = 8: 4 link stages + 2 z/t hop stages 0.69 ms; 8 + 2: 0.72; 4 + 3: 0.74 -- deeper rings do
+    // not help, the shared-memory port does the limiting
+    const char *zenv = getenv("BKR_WIN_NZ"), *lenv = getenv("BKR_WIN_RL");
+    int rl = lenv ? atoi(lenv) : 4, nz = zenv ? atoi(zenv) : 2;
+    if (rl != 4 && rl != 8) rl = 4;
+    if (nz != 1 && nz != 2 && nz != 4) nz = 2;
+    while (rl * lstage + wbytes + nz * zstage + rbytes + bbytes > WIN_SMEM_MAX) {
+        if (nz > 2) nz /= 2;
+        else if (rl > 4) rl = 4;
+        else if (nz > 1) nz /= 2;
+        else return 1;
+    }
+    if (nz < 2 && !getenv("BKR_WIN_ALLOW_NZ1")) return 1; // one z/t stage: slower than dslash.cu (48^4: 2.6 vs 2.1 ms)
+    p.nzlog = nz == 4 ? 2 : nz == 2 ? 1 : 0;
+    p.rllog = rl == 8 ? 3 : 2;
+    const size_t lbytes = rl * lstage;
     p.off_win = (uint32_t)lbytes;
     p.off_zt = (uint32_t)(lbytes + wbytes);
-    p.off_red = (uint32_t)(p.off_zt + (zstage << nzlog));
+    p.off_red = (uint32_t)(p.off_zt + nz * zstage);
     p.off_bar = (uint32_t)(p.off_red + rbytes);
     const size_t smem = p.off_bar + bbytes;
 
@@ -605,7 +621,7 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     }
     if (max_clusters == 0) return 1;
     if (getenv("BKR_WIN_DEBUG"))
-        fprintf(stderr, "dslash_win: C=%d max_clusters=%d nseg=%d smem=%zu WCH=%d nzlog=%d\n", C, max_clusters, p.nseg, smem, p.WCH, p.nzlog);
+        fprintf(stderr, "dslash_win: C=%d max_clusters=%d nseg=%d smem=%zu WCH=%d nz=%d rl=%d\n", C, max_clusters, p.nseg, smem, p.WCH, nz, rl);
     cfg.gridDim = dim3((unsigned)(std::min(max_clusters, p.nseg) * C));
     cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tm_win, tm_zt, p);
     if (e != cudaSuccess) {
@@ -624,17 +640,24 @@ int launch_dslash_win(bkr_ctx *ctx, int out_parity, int N, int prec, const void 
     const Geom &g = ctx->g;
     const int Xh = g.X[0] / 2;
     if (mode == 0 || (Xh * g.X[1]) % 64 != 0) return 1;
+    // Automatic mode: a cluster of C CTAs costs about C times the NC-rhs kernel whatever N is, the plain kernel of
+    // dslash.cu costs ~N; measured crossover at 32^3 x 64: within 2 rhs (fp64) / 3 rhs (fp32) of
+    // a full cluster.
     if (prec == BKR_F64) {
-        if (mode == 1 && N < 6) return 1;
         const int C = (N + 7) / 8;
+        if (mode == 1 && (N < 7 || 8 * C - N > 2)) return 1;
+        if (getenv("BKR_WIN_T8")) { // tuning probe
+            if (C == 1) return launch_win_c<double, 8, 1, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
+            if (C == 2) return launch_win_c<double, 8, 1, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
+        }
         if (C == 1) return launch_win_c<double, 4, 2, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
         if (C == 2) return launch_win_c<double, 4, 2, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
         if (C == 3) return launch_win_c<double, 4, 2, 3>(ctx, out_parity, N, prec, in, out, xp, a, done);
         if (C == 4) return launch_win_c<double, 4, 2, 4>(ctx, out_parity, N, prec, in, out, xp, a, done);
         return 1;
     }
-    if (mode == 1 && N < 12) return 1;
     const int C = (N + 15) / 16;
+    if (mode == 1 && (N < 13 || 16 * C - N > 3)) return 1;
     if (C == 1) return launch_win_c<float, 8, 2, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
     if (C == 2) return launch_win_c<float, 8, 2, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
     return 1;
