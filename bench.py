@@ -193,6 +193,8 @@ def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
     ms = time_loop(torch, f_dslash, reps, warmup)
     by, fl = bytes_dslash(dims, N, w), flops_dslash(dims, N)
     out["dslash"] = roofline_entry(ms, by, fl, hbm, prec == binding.F64)
+    out["dslash"]["variant"] = {0: "dslash_kernel (register tiling + link ring)",
+                                1: "dslash_win_kernel (shared-memory window, cluster-multicast links)"}.get(ctx.dslash_variant(), "?")
 
     def f_gram2():
         s, d = rot()
@@ -411,7 +413,7 @@ def run_bkr(args):
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "frac_hbm_iteration": value / world / hbm,
         "GFLOPS_iteration": world * flops_iteration(dims, N) / ms_step * 1e-6,
-        "roofline": {"bound": "hbm", "kernel": "dslash_kernel (multi-rhs Dslash, one parity, N=%d)" % N,
+        "roofline": {"bound": "hbm", "kernel": "%s: multi-rhs Dslash, one parity, N=%d" % (d.get("variant", "dslash"), N),
                      "achieved": d["GBps"], "peak": hbm, "unit": "GB/s", "frac": d["GBps"] / hbm,
                      "traffic": NCU_TRAFFIC.get((args.workload, N, "f64" if prec == binding.F64 else "f32")),
                      "frac_roofline": d["frac_roofline"], "binding": d["binding"],

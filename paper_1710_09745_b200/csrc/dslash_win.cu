@@ -134,7 +134,8 @@ template <typename Real, typename Cx> __device__ __forceinline__ void cfma3(Real
 // Inside a set, warp w handles rhs group w / 2 (T rhs) and sites (w % 2) * 32 + lane of the 64-site tile.
 template <typename Real, int T, int G, int C>
 __global__ void __launch_bounds__((4 * G + 3) * 32, 1)
-dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_constant__ CUtensorMap tm_zt, const WinParams p)
+dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_constant__ CUtensorMap tm_zt,
+                  const __grid_constant__ CUtensorMap tm_xp, const WinParams p)
 {
     typedef typename CxT<Real>::type Cx;
     constexpr int NC = T * G;
@@ -179,6 +180,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
     const int Xh = g.X[0] >> 1;
     const int Vh = g.Vh;
 
+    const int npt = p.xp ? 9 : 8; // z/t ring stages per tile: 8 hops + the xp tile of the epilogue
     const bool dry = (p.opts & 4) != 0; // tuning probe: no producers, no barriers (results are garbage)
     if (warp >= 2 * NWS) {
         // ------------------------------------------------------------------ producers: one lane in each of 3 warps
@@ -223,12 +225,13 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 for (int k = sg.x; k < sg.y; k++, tc++) {
                     const int knext = k + 1 < sg.y ? k + 1 : (has_next ? sn.x : -1); // this CTA's next tile
                     if (role == 2) {
-                        for (int j = 0; j < 8; j++) {
-                            const int zs = 8 * tc + j, slot = zs & (NZ - 1), use = zs >> nzlog;
+                        for (int j = 0; j < npt; j++) {
+                            const int zs = npt * tc + j, slot = zs & (NZ - 1), use = zs >> nzlog;
                             if (use > 0) mbar_wait(&zempty[slot], (use - 1) & 1);
                             mbar_expect_tx(&zfull[slot], ZSTAGE);
-                            tma_load_3d(zt + (size_t)slot * ZSTAGE, &tm_zt, 2 * zt_src(k, 8 + j), 0, (int)rank * NC, &zfull[slot]);
-                            if (knext >= 0 && (p.opts & 2)) tma_prefetch_3d(&tm_zt, 2 * zt_src(knext, 8 + j), 0, (int)rank * NC);
+                            if (j < 8) tma_load_3d(zt + (size_t)slot * ZSTAGE, &tm_zt, 2 * zt_src(k, 8 + j), 0, (int)rank * NC, &zfull[slot]);
+                            else tma_load_3d(zt + (size_t)slot * ZSTAGE, &tm_xp, 2 * k * 64, 0, (int)rank * NC, &zfull[slot]);
+                            if (j < 8 && knext >= 0 && (p.opts & 2)) tma_prefetch_3d(&tm_zt, 2 * zt_src(knext, 8 + j), 0, (int)rank * NC);
                         }
                         continue;
                     }
@@ -380,6 +383,8 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
         for (int si = cid; si < p.nseg; si += ncl) {
             const int4 sg = p.segs[si];
             for (int k = sg.x; k < sg.y; k++, tc++) {
+                const int e = k * 64 + sl;
+                Cx *vout = reinterpret_cast<Cx *>(p.out) + (size_t)jg * 3 * Vh + e;
                 Real acc[T][6];
 #pragma unroll
                 for (int i = 0; i < T; i++)
@@ -401,7 +406,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         else
                             for (uint32_t r = 0; r < (uint32_t)C; r++) mbar_arrive_remote(&lempty[slot], r);
                     }
-                    const int zs = 8 * tc + j, zslot = zs & (NZ - 1);
+                    const int zs = npt * tc + j, zslot = zs & (NZ - 1);
                     const Cx *zp = reinterpret_cast<const Cx *>(zt + (size_t)zslot * ZSTAGE) + j0 * 3 * 64 + sl;
                     if (!dry) mbar_wait(&zfull[zslot], (zs >> nzlog) & 1);
 #pragma unroll
@@ -417,36 +422,32 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         for (int i = 0; i < T; i++) cfma3<Real, Cx>(acc[i], u[b], v[i]);
                     }
                 }
-                const int e = k * 64 + sl;
-                Cx *vout = reinterpret_cast<Cx *>(p.out) + (size_t)jg * 3 * Vh + e;
-                const Cx *vxp = p.xp ? reinterpret_cast<const Cx *>(p.xp) + (size_t)jg * 3 * Vh + e : nullptr;
+                // xp operand of the epilogue: a ninth stage of the z/t ring (the producer copies the tile of xp behind
+                // the eight neighbour stages), so no arithmetic warp ever waits on global memory.  (With 3 T plain loads
+                // here the second half of M ran 1.83 ms against 1.38 ms for the bare stencil.)
+                const int zsx = npt * tc + 8, zslotx = zsx & (NZ - 1);
+                const Cx *zpx = reinterpret_cast<const Cx *>(zt + (size_t)zslotx * ZSTAGE) + j0 * 3 * 64 + sl;
+                if (p.xp && !dry) mbar_wait(&zfull[zslotx], (zsx >> nzlog) & 1);
                 if (!dry) mbar_wait_mem(redfull, tc & 1);
 #pragma unroll
-                for (int i = 0; i < T; i++)
+                for (int i = 0; i < T; i++) {
 #pragma unroll
                     for (int cc = 0; cc < 3; cc++) {
                         const Cx rb = red[((j0 + i) * 3 + cc) * 64 + sl];
-                        acc[i][2 * cc] += rb.x;
-                        acc[i][2 * cc + 1] += rb.y;
-                    }
-                if (!dry) mbar_arrive_mem(redempty);
-#pragma unroll
-                for (int i = 0; i < T; i++) {
-                    if (jg + i < p.N) {
-#pragma unroll
-                        for (int cc = 0; cc < 3; cc++) {
-                            Cx o;
-                            o.x = acc[i][2 * cc];
-                            o.y = acc[i][2 * cc + 1];
-                            if (vxp) {
-                                const Cx xv = __ldg(vxp + (size_t)(i * 3 + cc) * Vh);
-                                o.x = fma((Real)p.a, xv.x, -o.x);
-                                o.y = fma((Real)p.a, xv.y, -o.y);
-                            }
-                            __stcs(vout + (size_t)(i * 3 + cc) * Vh, o);
+                        Cx o;
+                        o.x = acc[i][2 * cc] + rb.x;
+                        o.y = acc[i][2 * cc + 1] + rb.y;
+                        if (p.xp) {
+                            const Cx xv = lds_cx(zpx + (i * 3 + cc) * 64);
+                            o.x = fma((Real)p.a, xv.x, -o.x);
+                            o.y = fma((Real)p.a, xv.y, -o.y);
                         }
+                        if (jg + i < p.N) __stcs(vout + (size_t)(i * 3 + cc) * Vh, o);
                     }
                 }
+                if (!dry) mbar_arrive_mem(redempty);
+                __syncwarp();
+                if (p.xp && lane == 0 && !dry) mbar_arrive(&zempty[zslotx]);
             }
         }
     }
@@ -575,8 +576,10 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
 
     const char *senv = getenv("BKR_WIN_SEGLEN");
     BKR_TRY(build_segments(ctx, N, prec, senv ? std::max(1, atoi(senv)) : 4));
-    CUtensorMap tm_win, tm_zt;
-    if (!make_map(&tm_win, in, prec, g.Vh, N, WIN_CHUNK, 3, NC) || !make_map(&tm_zt, in, prec, g.Vh, N, 64, 3, NC)) return 1;
+    CUtensorMap tm_win, tm_zt, tm_xp;
+    if (!make_map(&tm_win, in, prec, g.Vh, N, WIN_CHUNK, 3, NC) || !make_map(&tm_zt, in, prec, g.Vh, N, 64, 3, NC) ||
+        !make_map(&tm_xp, xp ? xp : in, prec, g.Vh, N, 64, 3, NC))
+        return 1;
 
     const int ntiles = link_tiles(g);
     p.g = g;
@@ -623,7 +626,7 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     if (getenv("BKR_WIN_DEBUG"))
         fprintf(stderr, "dslash_win: C=%d max_clusters=%d nseg=%d smem=%zu WCH=%d nz=%d rl=%d\n", C, max_clusters, p.nseg, smem, p.WCH, nz, rl);
     cfg.gridDim = dim3((unsigned)(std::min(max_clusters, p.nseg) * C));
-    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tm_win, tm_zt, p);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tm_win, tm_zt, tm_xp, p);
     if (e != cudaSuccess) {
         ctx->last_cuda = (int)e;
         return BKR_ECUDA;
