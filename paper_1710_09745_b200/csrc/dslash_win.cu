@@ -132,7 +132,7 @@ template <typename Real, typename Cx> __device__ __forceinline__ void cfma3(Real
 
 // blockDim = (4 G + 3) warps: warps [0, 2G) = set A (x/y hops), [2G, 4G) = set B (z/t hops), last 3 warps = producers.
 // Inside a set, warp w handles rhs group w / 2 (T rhs) and sites (w % 2) * 32 + lane of the 64-site tile.
-template <typename Real, int T, int G, int C>
+template <typename Real, int T, int G, int C, bool XP>
 __global__ void __launch_bounds__((4 * G + 3) * 32, 1)
 dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_constant__ CUtensorMap tm_zt,
                   const __grid_constant__ CUtensorMap tm_xp, const WinParams p)
@@ -180,7 +180,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
     const int Xh = g.X[0] >> 1;
     const int Vh = g.Vh;
 
-    const int npt = p.xp ? 9 : 8; // z/t ring stages per tile: 8 hops + the xp tile of the epilogue
+    constexpr int npt = XP ? 9 : 8; // z/t ring stages per tile: 8 hops + the xp tile of the epilogue
     const bool dry = (p.opts & 4) != 0; // tuning probe: no producers, no barriers (results are garbage)
     if (warp >= 2 * NWS) {
         // ------------------------------------------------------------------ producers: one lane in each of 3 warps
@@ -427,7 +427,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 // here the second half of M ran 1.83 ms against 1.38 ms for the bare stencil.)
                 const int zsx = npt * tc + 8, zslotx = zsx & (NZ - 1);
                 const Cx *zpx = reinterpret_cast<const Cx *>(zt + (size_t)zslotx * ZSTAGE) + j0 * 3 * 64 + sl;
-                if (p.xp && !dry) mbar_wait(&zfull[zslotx], (zsx >> nzlog) & 1);
+                if (XP && !dry) mbar_wait(&zfull[zslotx], (zsx >> nzlog) & 1);
                 if (!dry) mbar_wait_mem(redfull, tc & 1);
 #pragma unroll
                 for (int i = 0; i < T; i++) {
@@ -437,7 +437,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         Cx o;
                         o.x = acc[i][2 * cc] + rb.x;
                         o.y = acc[i][2 * cc + 1] + rb.y;
-                        if (p.xp) {
+                        if (XP) {
                             const Cx xv = lds_cx(zpx + (i * 3 + cc) * 64);
                             o.x = fma((Real)p.a, xv.x, -o.x);
                             o.y = fma((Real)p.a, xv.y, -o.y);
@@ -447,7 +447,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 }
                 if (!dry) mbar_arrive_mem(redempty);
                 __syncwarp();
-                if (p.xp && lane == 0 && !dry) mbar_arrive(&zempty[zslotx]);
+                if (XP && lane == 0 && !dry) mbar_arrive(&zempty[zslotx]);
             }
         }
     }
@@ -536,8 +536,8 @@ static const size_t WIN_SMEM_MAX = 232448;
 static int HcLextra(int HcL) { (void)HcL; return 2; } // 227 KB opt-in limit per CTA
 
 // returns 1 if this instantiation cannot run the geometry (caller falls back), BKR_OK after a launch, else an error
-template <typename Real, int T, int G, int C>
-static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *in, void *out, const void *xp, double a,
+template <typename Real, int T, int G, int C, bool XP>
+static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *in, void *out, const void *xp, double a,
                         const int *done)
 {
     typedef typename CxT<Real>::type Cx;
@@ -597,7 +597,7 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
         p.opts = oenv ? atoi(oenv) : 0;
     }
 
-    auto kern = dslash_win_kernel<Real, T, G, C>;
+    auto kern = dslash_win_kernel<Real, T, G, C, XP>;
     static int max_clusters = -1; // per instantiation
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
@@ -632,6 +632,14 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
         return BKR_ECUDA;
     }
     return bkr_check_launch(ctx);
+}
+
+template <typename Real, int T, int G, int C>
+static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *in, void *out, const void *xp, double a,
+                        const int *done)
+{
+    if (xp) return launch_win_x<Real, T, G, C, true>(ctx, parity, N, prec, in, out, xp, a, done);
+    return launch_win_x<Real, T, G, C, false>(ctx, parity, N, prec, in, out, xp, a, done);
 }
 
 // 1 = not applicable (caller uses dslash.cu's kernel)
