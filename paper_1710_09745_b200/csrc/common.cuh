@@ -40,6 +40,9 @@ struct SolverFlags {
     int want_update;   // mixed precision: reliable update requested (Alg. 3)
     double relres_max; // max_i ||C[:,i]|| / ||b_i||  after the last l.12
     double relres_last_update;
+    // deferred X update: xpend = 1 while W = beta C of the last l.9 has not been applied to X yet;
+    // xidle = !xpend (a kernel gate is "skip when the flag is non-zero", so the flush needs the negation)
+    int xpend, xidle;
 };
 
 struct bkr_ctx {
@@ -125,6 +128,12 @@ int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, dou
 // precZ is the precision of Z and C, precW of W; arithmetic in precZ.
 int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C,
                         const void *W, void *Z, const int *done);
+// Deferred X update fused with the P update (Alg. 1 l.10 of the previous iteration + l.8 of this one):
+//   if (flags->xpend)  X  += P Wm          (X fp64, in place)
+//   if (!flags->done)  Pn  = Q + P Sdag    (Pn must not alias P)
+// one pass over P for both products.  prec = precision of P, Q, Pn.
+int launch_px_update(bkr_ctx *ctx, int N, int prec, const double2 *Sdag, const double2 *Wm, const void *Q, const void *P,
+                     void *Pn, double2 *X, const SolverFlags *flags);
 // per-column reductions (two-stage, deterministic), results in out[j], j < N (device fp64):
 //   mode 0: sum_k |x_kj|^2        mode 1: Re sum_k conj(x_kj) y_kj      mode 2: sum_k |x_kj - y_kj|^2
 int launch_col_reduce(bkr_ctx *ctx, int N, int prec, int mode, const void *X, const void *Y, double *out,

@@ -148,7 +148,13 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
     __shared__ double scratch[BKR_MAX_N];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     SolverFlags *fl = p.flags;
-    if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) return;
+    if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) {
+        if (p.mode == SMALL_BETA && threadIdx.x == 0) { // no new W: nothing left to apply to X after this iteration
+            fl->xpend = 0;
+            fl->xidle = 1;
+        }
+        return;
+    }
 
     load_hermitian(p, A);
     if (warp == 0) {
@@ -164,6 +170,10 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
             if (fl) {
                 fl->breakdown = 1;
                 fl->done = 1;
+                if (p.mode == SMALL_BETA) {
+                    fl->xpend = 0;
+                    fl->xidle = 1;
+                }
             }
         }
         return;
@@ -209,6 +219,10 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
                 s.y += t.y;
             }
             p.W[o] = s;
+        }
+        if (threadIdx.x == 0 && fl) { // W is valid and not yet applied to X
+            fl->xpend = 1;
+            fl->xidle = 0;
         }
         break;
     }

@@ -158,6 +158,32 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
     return launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr);
 }
 
+// BKR_NO_DEFER=1 (comparison runs): X update as its own kernel right after l.9, as in the unfused Algorithm 1
+static bool defer_x()
+{
+    static const bool d = getenv("BKR_NO_DEFER") == nullptr;
+    return d;
+}
+
+// flags as the loop expects them after (re)initialisation: nothing pending for X
+static int reset_flags(bkr_ctx *ctx, Workspace *w)
+{
+    BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+    BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xidle, 1, sizeof(int), ctx->stream)); // any non-zero value
+    return BKR_OK;
+}
+
+// apply the deferred X += P (beta C) of the last completed l.9, if there is one (before X is read: loop exit,
+// reliable update)
+static int flush_x(bkr_ctx *ctx, Workspace *w)
+{
+    if (!defer_x()) return BKR_OK;
+    BKR_TRY(launch_block_update(ctx, w->N, BKR_F64, w->prec, w->W, w->Xn, w->P, w->Xn, &w->flags->xidle));
+    BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xpend, 0, sizeof(int), ctx->stream));
+    BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xidle, 1, sizeof(int), ctx->stream));
+    return BKR_OK;
+}
+
 // one iteration, Alg. 1 l.8-l.12
 static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, double delta, bool mixed)
 {
@@ -165,15 +191,21 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     const int *done = &w->flags->done;
     int np = 0;
     void *t;
-    // l.8  P = Q + P S^dag
-    BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done));
+    const bool defer = defer_x();
+    if (defer) {
+        // l.8  P = Q + P S^dag, fused with l.10 of the PREVIOUS iteration, X += P_old (beta C)_old: one pass over P for
+        // both (the deferral of PAPER.md:243).  flags->xpend says whether a W is waiting; flush_x() applies the last one.
+        BKR_TRY(launch_px_update(ctx, N, pr, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
+    } else {
+        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done));
+    }
     t = w->P; w->P = w->P2; w->P2 = t;
-    // l.9  beta = (P^dag M P)^-1
+    // l.9  beta = (P^dag M P)^-1 ; W = beta C
     BKR_TRY(apply_M(ctx, mass, N, pr, w->P, w->AP, done));
     BKR_TRY(launch_gram_partials(ctx, N, pr, w->P, w->AP, 1, &np, done));
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_BETA, np, tol, delta, mixed, ctx)));
-    // l.10 X = X + P (beta C)     (X in fp64 also in the mixed solver)
-    BKR_TRY(launch_block_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done));
+    // l.10 X = X + P (beta C)     (X in fp64 also in the mixed solver): deferred, see above
+    if (!defer) BKR_TRY(launch_block_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done));
     // l.11 Q S = Q - (M P) beta   (thin QR = Gram + Cholesky + scale, Algorithm 2)
     BKR_TRY(launch_block_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done));
     BKR_TRY(launch_gram_partials(ctx, N, pr, w->Q, w->Q, 1, &np, done));
@@ -221,7 +253,7 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
     double true_max = 0.0, iter_max = 0.0;
     const int check_every = mixed ? 1 : 8;
     for (;;) {
-        BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+        BKR_TRY(reset_flags(ctx, w));
         // l.3-l.6: R = B - M X ; Q C = R ; S = 1 ; P = 0
         BKR_TRY(block_residual_qr(ctx, w, mass, mixed ? w->Y : w->Xn, SMALL_INIT, tol, delta, mixed, nullptr));
         BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
@@ -234,6 +266,7 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
             iters = base + w->h_flags->iters;
             if (mixed && w->h_flags->want_update && !w->h_flags->done) {
                 // Algorithm 3: Y += X ; X = 0 ; R = B - M Y (fp64) ; Qhat C_new = R ; S = C_new Cprev^-1
+                BKR_TRY(flush_x(ctx, w));
                 BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, w->Y, 1.0, w->Xn, w->Y, nullptr));
                 BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
                 BKR_TRY(block_residual_qr(ctx, w, mass, w->Y, SMALL_RELUPD, tol, delta, mixed, nullptr));
@@ -241,6 +274,7 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
                 BKR_TRY(read_flags(ctx, w));
             }
         }
+        BKR_TRY(flush_x(ctx, w));
         iter_max = w->h_flags->relres_max;
         if (mixed) { // result = Y + X
             BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, w->Y, 1.0, w->Xn, w->Y, nullptr));
@@ -382,7 +416,7 @@ int solver_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const do
         BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
         if (mixed) BKR_CUDA(ctx, cudaMemsetAsync(w->Y, 0, w->bytes64, ctx->stream));
         BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 0, w->Bn, nullptr, w->bnorm2, nullptr));
-        BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+        BKR_TRY(reset_flags(ctx, w));
         BKR_TRY(block_residual_qr(ctx, w, mass, mixed ? w->Y : w->Xn, SMALL_INIT, 0.0, 0.0, false, nullptr));
         BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
         w->bench_ready = true;
