@@ -119,6 +119,32 @@ def test_maxiter_reports_noconv(cfg1):
     assert st["status"] == binding.ENOCONV and st["iters"] == 8 and max(rr) > TOL
 
 
+@pytest.mark.parametrize("k", [1, 3, 9])
+def test_iterate_after_k_iterations_matches_oracle(cfg1, k):
+    """X after exactly k iterations (maxiter = k, not converged) equals the oracle's k-th iterate: the X update of
+    Alg. 1 l.10 is deferred into the next iteration's P update on the GPU and must be flushed when the
+    loop stops early -- a missing flush leaves X one iteration behind.  Iterates are basis independent (U16)."""
+    import oracle
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, B, ctx = cfg1
+    X, rr, st = ctx.solve_block(0.1, torch.from_numpy(B).cuda(), tol=TOL, maxiter=k)
+    assert st["status"] == binding.ENOCONV and st["iters"] == k
+    ro = oracle.block_cg(dims, fat, lng, 0.1, B, tol=TOL, maxiter=k)
+    assert ro["iters"] == k
+    assert _soldiff(X.cpu().numpy(), ro["X"]) <= 1e-10
+
+
+def test_mixed_iterate_flushes_deferred_update(cfg1):
+    """same check through the reliable-update path: Y += X must see the deferred update (Alg. 3)"""
+    import oracle
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, B, ctx = cfg1
+    X, rr, st = ctx.solve_block(0.1, torch.from_numpy(B).cuda(), tol=TOL, inner_prec=binding.F32, delta=0.1)
+    assert st["status"] == 0 and st["reliable_updates"] >= 1 and max(rr) <= TOL
+    tr = oracle.true_relres(dims, fat, lng, 0.1, B, X.cpu().numpy())
+    assert tr.max() <= TOL
+
+
 def test_host_buffer_entry_points(cfg1):
     from paper_1710_09745_b200 import binding
     dims, fat, lng, B, ctx = cfg1
