@@ -51,6 +51,7 @@ struct WinParams {
     int WCH;    // window ring slots (chunks)
     int nzlog;  // log2 of the z/t stage ring depth
     int rllog;  // log2 of the link ring depth (2 or 3)
+    int slim;   // 1: window without spare slots (chunks below the tile released after the y-3, y-1 hops)
     int opts;   // tuning bits (BKR_WIN_OPTS): 1 = L2 prefetch of the next tile's links, 2 = of its z/t stages (no gain measured)
     uint32_t off_win, off_zt, off_red, off_bar;
 };
@@ -130,10 +131,10 @@ template <typename Real, typename Cx> __device__ __forceinline__ void cfma3(Real
     }
 }
 
-// blockDim = (4 G + 3) warps: warps [0, 2G) = set A (x/y hops), [2G, 4G) = set B (z/t hops), last 3 warps = producers.
+// blockDim = (4 G + 4) warps: warps [0, 2G) = set A (x/y hops), [2G, 4G) = set B (z/t hops), last 4 warps = producers.
 // Inside a set, warp w handles rhs group w / 2 (T rhs) and sites (w % 2) * 32 + lane of the 64-site tile.
 template <typename Real, int T, int G, int C, bool XP>
-__global__ void __launch_bounds__((4 * G + 3) * 32, 1)
+__global__ void __launch_bounds__((4 * G + 4) * 32, 1)
 dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_constant__ CUtensorMap tm_zt,
                   const __grid_constant__ CUtensorMap tm_xp, const WinParams p)
 {
@@ -183,10 +184,11 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
     constexpr int npt = XP ? 9 : 8; // z/t ring stages per tile: 8 hops + the xp tile of the epilogue
     const bool dry = (p.opts & 4) != 0; // tuning probe: no producers, no barriers (results are garbage)
     if (warp >= 2 * NWS) {
-        // ------------------------------------------------------------------ producers: one lane in each of 3 warps
-        //   role 0: link stages of set A (even sequence numbers) and the window chunks
+        // ------------------------------------------------------------------ producers: one lane in each of 4 warps
+        //   role 0: link stages of set A (even sequence numbers)
         //   role 1: link stages of set B (odd sequence numbers)
-        //   role 2: z/t neighbour sub-stages
+        //   role 2: z/t neighbour stages (and the xp tile of the epilogue)
+        //   role 3: window chunks
         // Each ring has its own in-order issuer, so a full ring never blocks the refill of another one.  Every
         // stage is also requested into L2 one tile ahead (cp.async.bulk.prefetch.L2): the HBM latency is paid there,
         // the shared-memory rings only have to cover the L2 -> SM latency.
@@ -235,10 +237,9 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         }
                         continue;
                     }
-                    // window chunks (role 0): what the first tile of a segment needs at once; later tiles find theirs
-                    // loaded from the middle of the previous tile (slots released one tile ago, so this never waits
-                    // for the tile in progress)
-                    auto load_chunks = [&](int hi) {
+                    if (role == 3) {
+                        // window chunks, up to what the NEXT tile needs, as far ahead as free slots allow
+                        const int hi = min(2 * k + 3 + HcL, seg_hi);
                         while (next_c <= hi) {
                             if (wuse > 0) mbar_wait(&wempty[wslot], (wuse - 1) & 1);
                             mbar_expect_tx(&wfull[wslot], WCHUNK);
@@ -249,8 +250,11 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                                 wuse++;
                             }
                         }
-                    };
-                    if (role == 0 && k == sg.x) load_chunks(min(2 * k + 1 + HcL, seg_hi));
+                        if (k == sg.y - 1 && has_next) // first window of the next segment -> L2
+                            for (int cc = 2 * sn.x - HcL; cc <= 2 * sn.x + 1 + HcL; cc++)
+                                tma_prefetch_3d(&tm_win, 2 * chunk_site0(cc, 2 * sn.z, 2 * (sn.w - sn.z + 1)), 0, (int)rank * NC);
+                        continue;
+                    }
                     for (int j = 0; j < 8; j++) {
                         const int h = role ? 8 + j : j;
                         const int ls = 16 * tc + 2 * j + role, slot = ls & (RL - 1), use = ls >> rllog;
@@ -264,12 +268,6 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                                            (uint16_t)((1u << C) - 1u), pol);
                         if (knext >= 0 && (p.opts & 1))
                             tma_prefetch_1d(reinterpret_cast<const unsigned char *>(wt + ((size_t)knext * 16 + h) * 9 * 64) + rank * SL, SL);
-                        if (role == 0 && j == 4) load_chunks(min(2 * k + 3 + HcL, seg_hi));
-                        if (role == 0 && j == 5 && k == sg.y - 1 && has_next) {
-                            // first window of the next segment -> L2
-                            for (int cc = 2 * sn.x - HcL; cc <= 2 * sn.x + 1 + HcL; cc++)
-                                tma_prefetch_3d(&tm_win, 2 * chunk_site0(cc, 2 * sn.z, 2 * (sn.w - sn.z + 1)), 0, (int)rank * NC);
-                        }
                     }
                 }
             }
@@ -348,6 +346,15 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                         for (int i = 0; i < T; i++) v[i] = lds_cx(wp + (i * 3 + b) * WIN_CHUNK);
 #pragma unroll
                         for (int i = 0; i < T; i++) cfma3<Real, Cx>(acc[i], u[b], v[i]);
+                    }
+                    if (h == 1 && p.slim) {
+                        // hops 0, 1 are y-3, y-1 (common.cuh): the chunks below the tile are dead from here on and go back
+                        // to the window producer, which loads the next tile's upper chunks into them
+                        const int new_rel = 2 * k;
+                        __syncwarp();
+                        if (lane == 0 && !dry)
+                            for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(q0 + cc - seg_lo) % WCH]);
+                        released = max(released, new_rel);
                     }
                 }
                 // release the window chunks the next tile of this segment does not need
@@ -530,11 +537,6 @@ static int build_segments(bkr_ctx *ctx, int N, int prec, int seglen)
 }
 
 static const size_t WIN_SMEM_MAX = 232448;
-// window slots beyond the 2 HcL + 2 chunks a tile reads: two, for the next tile's new chunks.  (Reusing the slots
-// below the tile, which are dead after the y-3, y-1 hops, saves 24 KB but makes the link producer wait for set A in
-// the middle of every tile: measured 0.72 -> 0.69 ms at N = 8 with the two spare slots.)
-static int HcLextra(int HcL) { (void)HcL; return 2; } // 227 KB opt-in limit per CTA
-
 // returns 1 if this instantiation cannot run the geometry (caller falls back), BKR_OK after a launch, else an error
 template <typename Real, int T, int G, int C, bool XP>
 static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *in, void *out, const void *xp, double a,
@@ -547,7 +549,11 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     WinParams p;
     memset(&p, 0, sizeof(p));
     p.HcL = (3 * Xh + WIN_CHUNK - 1) / WIN_CHUNK;
-    p.WCH = 2 * p.HcL + 2 + HcLextra(p.HcL);
+    {
+        const char *e = getenv("BKR_WIN_SLIM");
+        p.slim = e ? atoi(e) : 1;
+    }
+    p.WCH = 2 * p.HcL + 2 + (p.slim ? (p.HcL >= 2 ? 0 : 2 - p.HcL) : 2);
     if (p.WCH > 16) return 1;
     const size_t lstage = (size_t)9 * 64 * sizeof(Cx), wbytes = (size_t)p.WCH * NC * 3 * WIN_CHUNK * sizeof(Cx),
                  zstage = (size_t)NC * 3 * 64 * sizeof(Cx), rbytes = (size_t)NC * 3 * 64 * sizeof(Cx), bbytes = 66 * 8;
@@ -555,8 +561,8 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     // measured at 32^3 x 64, N = 8: 4 link stages + 2 z/t hop stages 0.69 ms; 8 + 2: 0.72; 4 + 3: 0.74 -- deeper rings do
     // not help, the shared-memory port does the limiting
     const char *zenv = getenv("BKR_WIN_NZ"), *lenv = getenv("BKR_WIN_RL");
-    int rl = lenv ? atoi(lenv) : 4, nz = zenv ? atoi(zenv) : 2;
-    if (rl != 4 && rl != 8) rl = 4;
+    int rl = lenv ? atoi(lenv) : 8, nz = zenv ? atoi(zenv) : 2;
+    if (rl != 4 && rl != 8) rl = 8;
     if (nz != 1 && nz != 2 && nz != 4) nz = 2;
     while (rl * lstage + wbytes + nz * zstage + rbytes + bbytes > WIN_SMEM_MAX) {
         if (nz > 2) nz /= 2;
@@ -575,7 +581,7 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     const size_t smem = p.off_bar + bbytes;
 
     const char *senv = getenv("BKR_WIN_SEGLEN");
-    BKR_TRY(build_segments(ctx, N, prec, senv ? std::max(1, atoi(senv)) : 4));
+    BKR_TRY(build_segments(ctx, N, prec, senv ? std::max(1, atoi(senv)) : 8));
     CUtensorMap tm_win, tm_zt, tm_xp;
     if (!make_map(&tm_win, in, prec, g.Vh, N, WIN_CHUNK, 3, NC) || !make_map(&tm_zt, in, prec, g.Vh, N, 64, 3, NC) ||
         !make_map(&tm_xp, xp ? xp : in, prec, g.Vh, N, 64, 3, NC))
@@ -606,7 +612,7 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     attr[0].val.clusterDim.x = C;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
-    cfg.blockDim = dim3((4 * G + 3) * 32);
+    cfg.blockDim = dim3((4 * G + 4) * 32);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->stream;
     cfg.attrs = attr;
