@@ -36,6 +36,10 @@
 #include <vector>
 
 #define WIN_CHUNK 32 /* sites per window chunk */
+#ifndef WIN_HOP_UNROLL
+#define WIN_HOP_UNROLL 1
+#endif
+static constexpr int HOP_UNROLL = WIN_HOP_UNROLL; // hop loops of the arithmetic warps (2 and 8 measured: no gain)
 
 struct WinParams {
     Geom g;
@@ -308,7 +312,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 for (int i = 0; i < T; i++)
 #pragma unroll
                     for (int qd = 0; qd < 6; qd++) acc[i][qd] = (Real)0;
-#pragma unroll 1
+#pragma unroll HOP_UNROLL
                 for (int h = 0; h < 8; h++) {
                     const int mu = BKR_HOP_MU(h), hop = BKR_HOP_LONG(h) ? 3 : 1;
                     const int cm = mu == 0 ? c0 : c1, Xm = mu == 0 ? g.X[0] : g.X[1], smh = mu == 0 ? 1 : g.X[0];
@@ -397,7 +401,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                 for (int i = 0; i < T; i++)
 #pragma unroll
                     for (int qd = 0; qd < 6; qd++) acc[i][qd] = (Real)0;
-#pragma unroll 1
+#pragma unroll HOP_UNROLL
                 for (int j = 0; j < 8; j++) {
                     const int ls = 16 * tc + 2 * j + 1, slot = ls & (RL - 1);
                     const Cx(*lk)[64] = reinterpret_cast<const Cx(*)[64]>(lnk + (size_t)slot * LSTAGE);
