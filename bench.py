@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- measurement harness.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl bkr|reference] [--workload cfg3|cfg5|cfg2]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl bkr|reference] [--workload cfg3|cfg4|cfg5|cfg2]
                     [--no-solve] [--sweep]
 
 A "step" is one blockCGrQ iteration (Algorithm 1 l.8-l.12 of arXiv:1710.09745: 2 multi-rhs Dslash, 2 Gram
@@ -35,6 +35,7 @@ WORKLOADS = {
     # name: (BASELINE.json config, dims, link kind, mass, N)
     "cfg2": ("configs[1]: 16^4, N=8, m=0.05", (16, 16, 16, 16), "perturbed", 0.05, 8),
     "cfg3": ("configs[2]: 32^3x64, N=16, m=0.01", (32, 32, 32, 64), "perturbed", 0.01, 16),
+    "cfg4": ("configs[3]: 48^3x96, N=32, m=0.005", (48, 48, 48, 96), "perturbed", 0.005, 32),
     "cfg5": ("configs[4]: 32^4 kernel sweep, N=16", (32, 32, 32, 32), "random", 0.05, 16),
 }
 

@@ -574,6 +574,12 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
         else if (nz > 1) nz /= 2;
         else return 1;
     }
+    {
+        // clusters of 3-4 CTAs need the deep link ring (the release -> refill round trip crosses SMs): with 4 stages the
+        // plain kernel is faster (48^3 x 96, N = 32 fp64: 20.6 vs 19.1 ms), with 8 it is not (32^3 x 64: 3.02 vs 3.10 ms)
+        const char *menv = getenv("BKR_DSLASH_WIN");
+        if (C >= 3 && rl < 8 && !(menv && atoi(menv) == 2)) return 1;
+    }
     if (nz < 2 && !getenv("BKR_WIN_ALLOW_NZ1")) return 1; // one z/t stage: slower than dslash.cu (48^4: 2.6 vs 2.1 ms)
     p.nzlog = nz == 4 ? 2 : nz == 2 ? 1 : 0;
     p.rllog = rl == 8 ? 3 : 2;
