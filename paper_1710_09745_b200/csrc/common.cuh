@@ -134,6 +134,10 @@ int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2
 // one pass over P for both products.  prec = precision of P, Q, Pn.
 int launch_px_update(bkr_ctx *ctx, int N, int prec, const double2 *Sdag, const double2 *Wm, const void *Q, const void *P,
                      void *Pn, double2 *X, const SolverFlags *flags);
+// The same with Alg. 2 l.4 of the previous iteration folded in (if !flags->done):  Q = Q Sinv (in place; Sinv upper
+// triangular, S^dag lower triangular: zero fragments skipped), Pn = Q + P Sdag;  X += P Wm if flags->xpend.
+int launch_pqx_update(bkr_ctx *ctx, int N, int prec, const double2 *Sinv, const double2 *Sdag, const double2 *Wm, void *Q,
+                      const void *P, void *Pn, double2 *X, const SolverFlags *flags);
 // per-column reductions (two-stage, deterministic), results in out[j], j < N (device fp64):
 //   mode 0: sum_k |x_kj|^2        mode 1: Re sum_k conj(x_kj) y_kj      mode 2: sum_k |x_kj - y_kj|^2
 int launch_col_reduce(bkr_ctx *ctx, int N, int prec, int mode, const void *X, const void *Y, double *out,

@@ -55,6 +55,7 @@ struct WinParams {
     int WCH;    // window ring slots (chunks)
     int nzlog;  // log2 of the z/t stage ring depth
     int rllog;  // log2 of the link ring depth (2 or 3)
+    int xover;  // 1: tiles do not start on x-row boundaries (64 % (X/2) != 0): x hops read the chunk below the tile
     int slim;   // 1: window without spare slots (chunks below the tile released after the y-3, y-1 hops)
     int opts;   // tuning bits (BKR_WIN_OPTS): 1 = L2 prefetch of the next tile's links, 2 = of its z/t stages (no gain measured)
     uint32_t off_win, off_zt, off_red, off_bar;
@@ -354,7 +355,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
                     if (h == 1 && p.slim) {
                         // hops 0, 1 are y-3, y-1 (common.cuh): the chunks below the tile are dead from here on and go back
                         // to the window producer, which loads the next tile's upper chunks into them
-                        const int new_rel = 2 * k;
+                        const int new_rel = 2 * k - p.xover; // x neighbours reach 2 sites below a tile that starts mid-row
                         __syncwarp();
                         if (lane == 0 && !dry)
                             for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(q0 + cc - seg_lo) % WCH]);
@@ -557,7 +558,8 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
         const char *e = getenv("BKR_WIN_SLIM");
         p.slim = e ? atoi(e) : 1;
     }
-    p.WCH = 2 * p.HcL + 2 + (p.slim ? (p.HcL >= 2 ? 0 : 2 - p.HcL) : 2);
+    p.xover = (64 % Xh) != 0 ? 1 : 0;
+    p.WCH = 2 * p.HcL + 2 + (p.slim ? std::max(0, 2 - (p.HcL - p.xover)) : 2);
     if (p.WCH > 16) return 1;
     const size_t lstage = (size_t)9 * 64 * sizeof(Cx), wbytes = (size_t)p.WCH * NC * 3 * WIN_CHUNK * sizeof(Cx),
                  zstage = (size_t)NC * 3 * 64 * sizeof(Cx), rbytes = (size_t)NC * 3 * 64 * sizeof(Cx), bbytes = 66 * 8;

@@ -143,6 +143,18 @@ static SmallArgs small_args(Workspace *w, int mode, int num_partials, double tol
     return a;
 }
 
+__global__ void set_identity_kernel(int N, double2 *A)
+{
+    for (int o = threadIdx.x; o < N * N; o += blockDim.x) A[o] = make_double2(o / N == o % N ? 1.0 : 0.0, 0.0);
+}
+
+// BKR_NO_QFUSE=1 (comparison runs): Q = Q' S^-1 as its own kernel at the end of the iteration
+static bool fuse_q()
+{
+    static const bool f = getenv("BKR_NO_QFUSE") == nullptr && getenv("BKR_NO_DEFER") == nullptr;
+    return f;
+}
+
 // Alg. 1 l.3-l.6 (and Alg. 3 l.4-l.6 when relupd): R = B - M Xcur in fp64, thin QR, Q in inner precision, P kept.
 static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const double2 *Xcur, int small_mode, double tol,
                              double delta, bool mixed, const int *gate)
@@ -155,7 +167,12 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
     BKR_TRY(launch_gram_partials(ctx, N, BKR_F64, w->R64, w->R64, 1, &np, gate));
     BKR_TRY(launch_small(ctx, small_args(w, small_mode, np, tol, delta, mixed, ctx)));
     // Q = R C^-1 (Alg. 2 l.4), stored in the inner precision
-    return launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr);
+    BKR_TRY(launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr));
+    if (fuse_q()) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
+        set_identity_kernel<<<1, 256, 0, ctx->stream>>>(N, w->Sinv);
+        BKR_TRY(bkr_check_launch(ctx));
+    }
+    return BKR_OK;
 }
 
 // BKR_NO_DEFER=1 (comparison runs): X update as its own kernel right after l.9, as in the unfused Algorithm 1
@@ -195,7 +212,9 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     if (defer) {
         // l.8  P = Q + P S^dag, fused with l.10 of the PREVIOUS iteration, X += P_old (beta C)_old: one pass over P for
         // both (the deferral of PAPER.md:243).  flags->xpend says whether a W is waiting; flush_x() applies the last one.
-        BKR_TRY(launch_px_update(ctx, N, pr, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
+        // With fuse_q() also Alg. 2 l.4 of the previous iteration, Q = Q' S^-1, in the same pass (Q' is read anyway).
+        if (fuse_q()) BKR_TRY(launch_pqx_update(ctx, N, pr, w->Sinv, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
+        else BKR_TRY(launch_px_update(ctx, N, pr, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
     } else {
         BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done));
     }
@@ -211,8 +230,10 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     BKR_TRY(launch_gram_partials(ctx, N, pr, w->Q, w->Q, 1, &np, done));
     // l.12 C = S C, residual norms, convergence / reliable-update flags
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_QR, np, tol, delta, mixed, ctx)));
-    BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done));
-    t = w->Q; w->Q = w->Q2; w->Q2 = t;
+    if (!fuse_q()) {
+        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done));
+        t = w->Q; w->Q = w->Q2; w->Q2 = t;
+    }
     return BKR_OK;
 }
 

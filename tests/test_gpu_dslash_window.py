@@ -21,7 +21,8 @@ LATTICES = {
     "16x16x4x6": (16, 16, 4, 6),    # two tiles per strip, reach 1 chunk
     "8x16x6x4": (8, 16, 6, 4),      # X/2 = 4: four rows per chunk
     "32x8x4x4": (32, 8, 4, 4),      # reach 2 chunks, strip shorter than the window
-    "32x32x4x8": (32, 32, 4, 8),    # 8 tiles per strip = two segments, the shape of configs 3 and 5
+    "32x32x4x8": (32, 32, 4, 8),    # 8 tiles per strip, the shape of configs 3 and 5
+    "48x16x4x4": (48, 16, 4, 4),    # X/2 = 24: tiles start mid-row (x hops reach below the tile), reach 3 chunks: config 4
 }
 
 
