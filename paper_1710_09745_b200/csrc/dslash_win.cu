@@ -516,7 +516,7 @@ static int build_segments(bkr_ctx *ctx, int N, int prec, int seglen)
     const int Xh = g.X[0] / 2, Y = g.X[1], Z = g.X[2], Tt = g.X[3];
     static const char *env = getenv("BKR_L2_BUDGET_MB");
     const double budget = (env ? atof(env) : 48.0) * 1e6;
-    const double site_bytes = 3.0 * N * (prec == BKR_F64 ? 16 : 8);
+    const double site_bytes = 3.0 * std::max(N, ctx->dslash_nblock) * (prec == BKR_F64 ? 16 : 8);
     int zb = 1;
     for (int c = 1; c <= Z; c++)
         if (Z % c == 0 && (7.0 * Xh * Y * c * site_bytes <= budget || Tt <= 7)) zb = c;
