@@ -155,7 +155,7 @@ SM_COUNT, SM_MAX_MHZ = 148, 1965.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
 # capture of this same bench command (profiles/r1_ncu_summary.md); None where no capture exists.
-NCU_TRAFFIC = {("cfg3", 16, "f64"): 4.220473e9 + 0.787975e9}
+NCU_TRAFFIC = {("cfg3", 16, "f64"): 4.501845e9 + 0.788309e9}
 
 
 def alu_peak_gflops(fp64):
