@@ -229,6 +229,9 @@ def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
 
 # ---------------------------------------------------------------- CPU baseline (the oracle, as it stands)
 
+_ORACLE_INPUTS = {}
+
+
 def oracle_sample(dims_full, N, kind, seed=5):
     """One blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update) with the oracle on a bounded
     sample: the same N and link generator on a lattice shrunk until it is ~10-30 s of CPU work.
@@ -241,10 +244,14 @@ def oracle_sample(dims_full, N, kind, seed=5):
         k = max(range(4), key=lambda mu: dims[mu])
         dims[k] //= 2
     dims = tuple(dims)
-    fat, lng = synth.make_links(dims, kind, seed)
-    fat, lng = fat.numpy(), lng.numpy()
-    P = synth.make_sources(dims, N, seed + 1).numpy()
-    Q = synth.make_sources(dims, N, seed + 2).numpy()
+    key = (dims, N, kind, seed)
+    if key not in _ORACLE_INPUTS:  # inputs are generated once per process, outside every timed step
+        fat, lng = synth.make_links(dims, kind, seed)
+        _ORACLE_INPUTS.clear()
+        _ORACLE_INPUTS[key] = (fat.numpy(), lng.numpy(), synth.make_sources(dims, N, seed + 1).numpy(),
+                               synth.make_sources(dims, N, seed + 2).numpy())
+    fat, lng, P, Q = _ORACLE_INPUTS[key]
+    Q = Q.copy()
     a = (np.eye(N) * 0.5).astype(np.complex128)
     oracle.lib()
     t0 = time.perf_counter()
@@ -271,7 +278,7 @@ def run_reference(args):
         dt, by, desc, threads = oracle_sample(dims, N, kind)
         if i >= args.warmup:
             times.append(dt)
-        if sum(times) > 150:
+        if sum(times) > 120:  # bounded: the whole run ends within a few minutes whatever --steps says
             break
     ms = 1e3 * sum(times) / len(times)
     val = by / ms * 1e-6
