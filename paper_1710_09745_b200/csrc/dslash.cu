@@ -351,12 +351,19 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
     // fp64 blocks of more than 16 rhs go through in chunks of 16: two cluster-of-2 window launches beat one cluster of 4
     // (32^3 x 64, N = 32: 2 x 1.32 ms against 3.02 ms; 48^3 x 96: 2 x 7.3 ms against 19.1 ms for the plain kernel) although
     // the links are then read once per chunk.  A chunk is a contiguous view of the native block [rhs][colour][site].
-    if (prec == BKR_F64 && N > 16 && !getenv("BKR_DSLASH_NOSPLIT")) {
-        const size_t stride = (size_t)3 * ctx->g.Vh * sizeof(double2);
+    // Likewise 11-13 rhs as 8 + rest (window kernel + plain kernel) and fp32 blocks of 17-28 rhs as 16 + rest.
+    int chunk = 0;
+    if (!getenv("BKR_DSLASH_NOSPLIT")) {
+        if (prec == BKR_F64 && N > 16) chunk = 16;
+        else if (prec == BKR_F64 && N >= 11 && N <= 13) chunk = 8; // 14 = window cluster of 2 (1.29 ms) beats 8 + 6 (1.32 ms)
+        else if (prec == BKR_F32 && N > 16 && N <= 28) chunk = 16;
+    }
+    if (chunk) {
+        const size_t stride = (size_t)3 * ctx->g.Vh * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
         ctx->dslash_nblock = N;
         int rc = BKR_OK;
-        for (int j = 0; j < N && rc == BKR_OK; j += 16) {
-            const int n = N - j < 16 ? N - j : 16;
+        for (int j = 0; j < N && rc == BKR_OK; j += chunk) {
+            const int n = N - j < chunk ? N - j : chunk;
             rc = launch_dslash(ctx, out_parity, n, prec, (const char *)in + j * stride, (char *)out + j * stride,
                                xp ? (const char *)xp + j * stride : nullptr, a, done);
         }
