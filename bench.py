@@ -415,7 +415,7 @@ def run_bkr(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == binding.F64 else "f32", "data": "synthetic",
         "config": {"workload": name, "dims": list(dims), "N": N, "mass": mass, "links": kind,
-                   "step": "one blockCGrQ iteration (Alg. 1 l.8-12): 2 Dslash, 2 Gram, fused Q+P+X update, Q' update, 2 small-matrix kernels",
+                   "step": "one blockCGrQ iteration (Alg. 1 l.8-12): 2 Dslash, Gram P^H MP, fused Q+P+X update, fused Q' update + Gram, 2 small-matrix kernels",
                    "l2": "inputs larger than L2 (links %.2f GB + blocks %.2f GB each)" % (
                        144 * w * volume(dims) * 1e-9, block_bytes(dims, N, w) * 1e-9),
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},

@@ -139,6 +139,9 @@ int launch_px_update(bkr_ctx *ctx, int N, int prec, const double2 *Sdag, const d
 // triangular, S^dag lower triangular: zero fragments skipped), Pn = Q + P Sdag;  X += P Wm if flags->xpend.
 int launch_pqx_update(bkr_ctx *ctx, int N, int prec, const double2 *Sinv, const double2 *Sdag, const double2 *Wm, void *Q,
                       const void *P, void *Pn, double2 *X, const SolverFlags *flags);
+// Alg. 1 l.11 + Alg. 2 l.2 fused: Z = C + W a and stage 1 of H = Z^dag Z (Hermitian) in one pass; all blocks precision prec.
+int launch_update_gram(bkr_ctx *ctx, int N, int prec, const double2 *a, const void *C, const void *W, void *Z, int *num_partials,
+                       const int *done);
 // per-column reductions (two-stage, deterministic), results in out[j], j < N (device fp64):
 //   mode 0: sum_k |x_kj|^2        mode 1: Re sum_k conj(x_kj) y_kj      mode 2: sum_k |x_kj - y_kj|^2
 int launch_col_reduce(bkr_ctx *ctx, int N, int prec, int mode, const void *X, const void *Y, double *out,

@@ -958,3 +958,218 @@ int launch_pqx_update(bkr_ctx *ctx, int N, int prec, const double2 *Sinv, const 
     if (prec == BKR_F64) return launch_pqx_t<double>(ctx, N, Sinv, Sdag, Wm, Q, P, Pn, X, flags);
     return launch_pqx_t<float>(ctx, N, Sinv, Sdag, Wm, Q, P, Pn, X, flags);
 }
+
+// ------------------------------------------------------------------------------------------ fused update + aliased Gram
+// Alg. 1 l.11 / Alg. 2 l.2 in one pass:  Z = C + W a  (Q' = Q - MP beta)  and  H = Z^dag Z  (Hermitian, upper
+// tile pairs).  The update part is update_tma_kernel's; each warp then writes its 8 finished rows of Z -- rounded to the
+// storage precision, so that H is the Gram matrix of what is stored -- over the C rows it has just consumed in the ring
+// and feeds them back as DMMA fragments of the reduction (gram_tma_kernel's tiles, accumulators and fixed-order
+// two-stage reduction).  Saves the separate read of Z.
+template <typename Real, int NT, int NIS, int CW>
+__global__ void __launch_bounds__((CW + 1) * 32, 1)
+update_gram_kernel(size_t L, int N, RingPlan rp, uint32_t off_red, const double2 *__restrict__ a,
+                   const typename CxT<Real>::type *C, const typename CxT<Real>::type *__restrict__ W,
+                   typename CxT<Real>::type *Z, double2 *__restrict__ partials, const int *done)
+{
+    typedef typename CxT<Real>::type Cx;
+    constexpr int NTJ = NT;
+    constexpr int NF = NIS * NTJ * 32;
+    constexpr int NP = NT * (NT + 1) / 2;
+    extern __shared__ __align__(128) unsigned char dsm[];
+    uint64_t *full = reinterpret_cast<uint64_t *>(dsm);
+    uint64_t *empty = full + MB_MAX_STAGES;
+    double *bre = reinterpret_cast<double *>(dsm + 128), *bim = bre + NF;
+    double2 *red = reinterpret_cast<double2 *>(dsm + off_red); // [N * N]
+    unsigned char *ring = dsm + rp.off_ring;
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < rp.nstg; s++) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], CW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int idx = threadIdx.x; idx < NF; idx += blockDim.x) {
+        const int ln = idx & 31, f = idx >> 5;
+        const int is = f / NTJ, tj = f % NTJ;
+        const int i = 4 * is + (ln & 3), j = 8 * tj + (ln >> 2);
+        const double2 v = (i < N && j < N) ? a[i * N + j] : make_double2(0.0, 0.0);
+        bre[idx] = v.x;
+        bim[idx] = v.y;
+    }
+    for (int o = threadIdx.x; o < N * N; o += blockDim.x) red[o] = make_double2(0.0, 0.0);
+    __syncthreads();
+
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const int my = (int)((ntiles > blockIdx.x) ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0);
+
+    if (warp == CW) { // ---------------- producer
+        const uint64_t pol = policy_evict_first();
+        for (int it = 0; it < my; it++) {
+            const int s = it % rp.nstg;
+            if (it >= rp.nstg) mbar_wait(&empty[s], ((it / rp.nstg) - 1) & 1);
+            const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
+            const uint32_t rows = (uint32_t)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
+            unsigned char *st = ring + (size_t)s * rp.stage_bytes;
+            if (lane == 0) mbar_expect_tx(&full[s], (uint32_t)N * rows * 2u * (uint32_t)sizeof(Cx));
+            __syncwarp();
+            if (lane < N) {
+                tma_load_1d_hint(st + (size_t)lane * rp.rs_a, W + (size_t)lane * L + r0, rows * (uint32_t)sizeof(Cx), &full[s], pol);
+                tma_load_1d_hint(st + rp.off_b + (size_t)lane * rp.rs_b, C + (size_t)lane * L + r0, rows * (uint32_t)sizeof(Cx),
+                                 &full[s], pol);
+            }
+        }
+        return;
+    }
+
+    // ---------------- consumers
+    const int m = lane >> 2, q = lane & 3;
+    double acc[NP][4][2]; // Zr Zr, Zr Zi, Zi Zr, Zi Zi per tile pair
+#pragma unroll
+    for (int p = 0; p < NP; p++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) acc[p][c][0] = acc[p][c][1] = 0.0;
+    for (int it = 0; it < my; it++) {
+        const int s = it % rp.nstg;
+        const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
+        const int rows = (int)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
+        const unsigned char *stW = ring + (size_t)s * rp.stage_bytes;
+        unsigned char *stC = ring + (size_t)s * rp.stage_bytes + rp.off_b;
+        mbar_wait_acq(&full[s], (it / rp.nstg) & 1);
+        for (int u = warp; u < rows / 8; u += CW) {
+            const int row = 8 * u + m;
+            double2 wf[NIS];
+#pragma unroll
+            for (int is = 0; is < NIS; is++) {
+                const int i = 4 * is + q;
+                wf[is] = i < N ? sm_cx<Cx>(stW + (size_t)i * rp.rs_a + (size_t)row * sizeof(Cx)) : make_double2(0.0, 0.0);
+            }
+            double zre[NTJ][2], zim[NTJ][2];
+#pragma unroll
+            for (int tj = 0; tj < NTJ; tj++) zre[tj][0] = zre[tj][1] = zim[tj][0] = zim[tj][1] = 0.0;
+#pragma unroll
+            for (int is = 0; is < NIS; is++)
+#pragma unroll
+                for (int tj = 0; tj < NTJ; tj++) {
+                    const int f = (is * NTJ + tj) * 32 + lane;
+                    const double br = bre[f], bi = bim[f];
+                    dmma(zre[tj], wf[is].x, br);
+                    dmma(zre[tj], wf[is].y, -bi);
+                    dmma(zim[tj], wf[is].x, bi);
+                    dmma(zim[tj], wf[is].y, br);
+                }
+#pragma unroll
+            for (int tj = 0; tj < NTJ; tj++)
+#pragma unroll
+                for (int r = 0; r < 2; r++) {
+                    const int j = 8 * tj + 2 * q + r;
+                    if (j < N) {
+                        Cx *cp = reinterpret_cast<Cx *>(stC + (size_t)j * rp.rs_b + (size_t)row * sizeof(Cx));
+                        const Cx c = *cp;
+                        Cx zv; // rounded to the storage precision: H is the Gram matrix of what is stored
+                        zv.x = (Real)(zre[tj][r] + (double)c.x);
+                        zv.y = (Real)(zim[tj][r] + (double)c.y);
+                        *cp = zv;
+                        __stcs(Z + (size_t)j * L + r0 + row, zv);
+                    }
+                }
+            __syncwarp();
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                double2 xf[NT];
+#pragma unroll
+                for (int t = 0; t < NT; t++)
+                    xf[t] = (8 * t + m) < N
+                                ? sm_cx<Cx>(stC + (size_t)(8 * t + m) * rp.rs_b + (size_t)(8 * u + 4 * h + q) * sizeof(Cx))
+                                : make_double2(0.0, 0.0);
+                int p = 0;
+#pragma unroll
+                for (int ti = 0; ti < NT; ti++)
+#pragma unroll
+                    for (int tj = ti; tj < NT; tj++, p++) {
+                        dmma(acc[p][0], xf[ti].x, xf[tj].x);
+                        dmma(acc[p][1], xf[ti].x, xf[tj].y);
+                        dmma(acc[p][2], xf[ti].y, xf[tj].x);
+                        dmma(acc[p][3], xf[ti].y, xf[tj].y);
+                    }
+            }
+        }
+        // generic-proxy writes to the stage before the async-proxy (TMA) refill of the same shared memory
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive_rel(&empty[s]);
+    }
+    for (int w = 0; w < CW; w++) { // fixed-order reduction over the consumer warps (named barrier 1: the producer has left)
+        if (warp == w) {
+            int p = 0;
+#pragma unroll
+            for (int ti = 0; ti < NT; ti++)
+#pragma unroll
+                for (int tj = ti; tj < NT; tj++, p++)
+#pragma unroll
+                    for (int r = 0; r < 2; r++) {
+                        const int i = 8 * ti + m, j = 8 * tj + 2 * q + r;
+                        if (i < N && j < N) {
+                            double2 v = red[i * N + j];
+                            v.x += acc[p][0][r] + acc[p][3][r];
+                            v.y += acc[p][1][r] - acc[p][2][r];
+                            red[i * N + j] = v;
+                        }
+                    }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(CW * 32) : "memory");
+    }
+    for (int o = threadIdx.x; o < N * N; o += CW * 32) partials[(size_t)blockIdx.x * N * N + o] = red[o];
+}
+
+template <typename Real, int NT, int NIS>
+static int update_gram_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const void *C, const void *W, void *Z, int *num_partials,
+                          const int *done)
+{
+    typedef typename CxT<Real>::type Cx;
+    constexpr int CW = 8;
+    const size_t off_red = (128 + (size_t)2 * NIS * NT * 32 * sizeof(double) + 127) / 128 * 128;
+    const size_t fixed = off_red + (size_t)N * N * sizeof(double2);
+    const RingPlan rp = plan_ring(L, fixed, 4, N, (int)sizeof(Cx), 32, N, (int)sizeof(Cx), 16);
+    if (rp.nstg < 2) return BKR_EINVAL;
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
+    BKR_TRY(ensure_partials(ctx, (size_t)2 * BKR_NUM_SMS * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
+    static bool attr_done = false; // one flag per instantiation
+    if (!attr_done) {
+        BKR_CUDA(ctx, cudaFuncSetAttribute(update_gram_kernel<Real, NT, NIS, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           MB_SMEM_BUDGET));
+        attr_done = true;
+    }
+    update_gram_kernel<Real, NT, NIS, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
+        L, N, rp, (uint32_t)off_red, a, (const Cx *)C, (const Cx *)W, (Cx *)Z, ctx->partials, done);
+    *num_partials = (int)grid;
+    return bkr_check_launch(ctx);
+}
+
+// Z = C + W a (Z may alias C) and per-CTA partials of the Hermitian Gram matrix Z^dag Z in ctx->partials (second stage:
+// small_kernel or launch_gram_finish, as after launch_gram_partials).  All blocks in precision prec.
+int launch_update_gram(bkr_ctx *ctx, int N, int prec, const double2 *a, const void *C, const void *W, void *Z, int *num_partials,
+                       const int *done)
+{
+    const size_t L = (size_t)ctx->g.Vh * 3;
+#define UG_GO(Real, NT_, NIS_) return update_gram_go<Real, NT_, NIS_>(ctx, L, N, a, C, W, Z, num_partials, done)
+#define UG_SW(Real)                  \
+    switch ((N + 3) / 4) {           \
+    case 1: UG_GO(Real, 1, 1);       \
+    case 2: UG_GO(Real, 1, 2);       \
+    case 3: UG_GO(Real, 2, 3);       \
+    case 4: UG_GO(Real, 2, 4);       \
+    case 5: UG_GO(Real, 3, 5);       \
+    case 6: UG_GO(Real, 3, 6);       \
+    case 7: UG_GO(Real, 4, 7);       \
+    default: UG_GO(Real, 4, 8);      \
+    }
+    if (prec == BKR_F64) {
+        UG_SW(double)
+    }
+    UG_SW(float)
+#undef UG_SW
+#undef UG_GO
+}

@@ -226,8 +226,13 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     // l.10 X = X + P (beta C)     (X in fp64 also in the mixed solver): deferred, see above
     if (!defer) BKR_TRY(launch_block_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done));
     // l.11 Q S = Q - (M P) beta   (thin QR = Gram + Cholesky + scale, Algorithm 2)
-    BKR_TRY(launch_block_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done));
-    BKR_TRY(launch_gram_partials(ctx, N, pr, w->Q, w->Q, 1, &np, done));
+    static const bool fuse_gram = getenv("BKR_NO_GRAMFUSE") == nullptr;
+    if (fuse_gram) { // one pass: Q' and stage 1 of H = Q'^dag Q'
+        BKR_TRY(launch_update_gram(ctx, N, pr, w->negbeta, w->Q, w->AP, w->Q, &np, done));
+    } else {
+        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done));
+        BKR_TRY(launch_gram_partials(ctx, N, pr, w->Q, w->Q, 1, &np, done));
+    }
     // l.12 C = S C, residual norms, convergence / reliable-update flags
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_QR, np, tol, delta, mixed, ctx)));
     if (!fuse_q()) {
