@@ -149,10 +149,14 @@ __global__ void set_identity_kernel(int N, double2 *A)
 }
 
 // BKR_NO_QFUSE=1 (comparison runs): Q = Q' S^-1 as its own kernel at the end of the iteration
-static bool fuse_q()
+// Fused updates only up to 24 rhs: beyond, the update kernels are bound by the FP64 tensor pipe, the fused ones spill,
+// and separate kernels are faster (32^4, N = 32: 5.39 vs 5.58 ms per iteration; N = 24: 3.82 vs 3.76 ms).
+static const int FUSE_MAX_N = 24;
+
+static bool fuse_q(int N)
 {
     static const bool f = getenv("BKR_NO_QFUSE") == nullptr && getenv("BKR_NO_DEFER") == nullptr;
-    return f;
+    return f && N <= FUSE_MAX_N;
 }
 
 // Alg. 1 l.3-l.6 (and Alg. 3 l.4-l.6 when relupd): R = B - M Xcur in fp64, thin QR, Q in inner precision, P kept.
@@ -168,7 +172,7 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
     BKR_TRY(launch_small(ctx, small_args(w, small_mode, np, tol, delta, mixed, ctx)));
     // Q = R C^-1 (Alg. 2 l.4), stored in the inner precision
     BKR_TRY(launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr));
-    if (fuse_q()) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
+    if (fuse_q(N)) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
         set_identity_kernel<<<1, 256, 0, ctx->stream>>>(N, w->Sinv);
         BKR_TRY(bkr_check_launch(ctx));
     }
@@ -176,10 +180,10 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
 }
 
 // BKR_NO_DEFER=1 (comparison runs): X update as its own kernel right after l.9, as in the unfused Algorithm 1
-static bool defer_x()
+static bool defer_x(int N)
 {
     static const bool d = getenv("BKR_NO_DEFER") == nullptr;
-    return d;
+    return d && N <= FUSE_MAX_N;
 }
 
 // flags as the loop expects them after (re)initialisation: nothing pending for X
@@ -194,7 +198,7 @@ static int reset_flags(bkr_ctx *ctx, Workspace *w)
 // reliable update)
 static int flush_x(bkr_ctx *ctx, Workspace *w)
 {
-    if (!defer_x()) return BKR_OK;
+    if (!defer_x(w->N)) return BKR_OK;
     BKR_TRY(launch_block_update(ctx, w->N, BKR_F64, w->prec, w->W, w->Xn, w->P, w->Xn, &w->flags->xidle));
     BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xpend, 0, sizeof(int), ctx->stream));
     BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xidle, 1, sizeof(int), ctx->stream));
@@ -208,12 +212,12 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     const int *done = &w->flags->done;
     int np = 0;
     void *t;
-    const bool defer = defer_x();
+    const bool defer = defer_x(N);
     if (defer) {
         // l.8  P = Q + P S^dag, fused with l.10 of the PREVIOUS iteration, X += P_old (beta C)_old: one pass over P for
         // both (the deferral of PAPER.md:243).  flags->xpend says whether a W is waiting; flush_x() applies the last one.
-        // With fuse_q() also Alg. 2 l.4 of the previous iteration, Q = Q' S^-1, in the same pass (Q' is read anyway).
-        if (fuse_q()) BKR_TRY(launch_pqx_update(ctx, N, pr, w->Sinv, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
+        // With fuse_q(N) also Alg. 2 l.4 of the previous iteration, Q = Q' S^-1, in the same pass (Q' is read anyway).
+        if (fuse_q(N)) BKR_TRY(launch_pqx_update(ctx, N, pr, w->Sinv, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
         else BKR_TRY(launch_px_update(ctx, N, pr, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
     } else {
         BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done));
@@ -227,7 +231,9 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     if (!defer) BKR_TRY(launch_block_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done));
     // l.11 Q S = Q - (M P) beta   (thin QR = Gram + Cholesky + scale, Algorithm 2)
     static const bool fuse_gram = getenv("BKR_NO_GRAMFUSE") == nullptr;
-    if (fuse_gram) { // one pass: Q' and stage 1 of H = Q'^dag Q'
+    // N <= 16 only: with 3-4 column tiles the reduction's 6-10 tile-pair accumulators no longer fit beside the update's
+    // (ptxas spills; measured 4.08 vs 3.76 ms per iteration at N = 24, 5.76 vs 5.58 at N = 32 on 32^4)
+    if (fuse_gram && N <= 16) { // one pass: Q' and stage 1 of H = Q'^dag Q'
         BKR_TRY(launch_update_gram(ctx, N, pr, w->negbeta, w->Q, w->AP, w->Q, &np, done));
     } else {
         BKR_TRY(launch_block_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done));
@@ -235,7 +241,7 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     }
     // l.12 C = S C, residual norms, convergence / reliable-update flags
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_QR, np, tol, delta, mixed, ctx)));
-    if (!fuse_q()) {
+    if (!fuse_q(N)) {
         BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done));
         t = w->Q; w->Q = w->Q2; w->Q2 = t;
     }
