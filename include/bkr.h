@@ -105,6 +105,12 @@ int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int he
  * streamed once.  a: N*N complex fp64; X, Y native, X != Y. */
 int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y);
 
+/* The two fused, as the solver uses them for Algorithm 1 l.11 + Algorithm 2 l.2 (aliased
+ * Hermitian reduction PAPER.md:289):  Y <- Y + X a  and  K = Y^dag Y  of the updated Y, in one pass over X and Y.
+ * K is the Gram matrix of Y as stored (for fp32 blocks: of the fp32-rounded result), accumulated in fp64, Hermitian
+ * with a real diagonal, bit-reproducible.  a, K: N*N complex fp64 (device); X, Y native, X != Y. */
+int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y, void *K);
+
 /* Small dense algebra on the device, one warp (Algorithm 2 l.3):
  * bkr_cholesky_upper: H = R^dag R, R upper triangular with real positive diagonal; Rinv = R^-1.
  * bkr_hpd_inverse   : Ginv = G^-1 for Hermitian positive-definite G (via Cholesky).

@@ -19,7 +19,7 @@ MAX_N = 32
 
 SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash",
-    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
+    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_axpy_gram", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
     "bkr_strerror", "bkr_version", "bkr_dslash_variant",
 )
@@ -65,6 +65,7 @@ def lib():
             "bkr_apply_M": (ci, [vp, cd, ci, ci, vp, vp]),
             "bkr_gram": (ci, [vp, ci, ci, vp, vp, ci, vp]),
             "bkr_block_axpy": (ci, [vp, ci, ci, vp, vp, vp]),
+            "bkr_block_axpy_gram": (ci, [vp, ci, ci, vp, vp, vp, vp]),
             "bkr_cholesky_upper": (ci, [vp, ci, vp, vp, vp, vp]),
             "bkr_hpd_inverse": (ci, [vp, ci, vp, vp, vp]),
             "bkr_solve_block": (ci, [vp, cd, ci, vp, vp, cd, ci, ci, cd, vp, ctypes.POINTER(Stats)]),
@@ -184,6 +185,14 @@ class Context:
         self._check(lib().bkr_block_axpy(self._h, int(N), int(prec), _dev_ptr(a, "a"), _dev_ptr(X, "X"), _dev_ptr(Y, "Y")),
                     "bkr_block_axpy")
         return Y
+
+    def block_axpy_gram(self, N, a, X, Y, prec=F64, out=None):
+        """Y += X a and K = Y^dag Y of the updated Y in one pass; returns K (N x N complex128)."""
+        assert a.dtype == torch.complex128 and tuple(a.shape) == (int(N), int(N))
+        K = out if out is not None else torch.empty(int(N), int(N), dtype=torch.complex128, device=self.device)
+        self._check(lib().bkr_block_axpy_gram(self._h, int(N), int(prec), _dev_ptr(a, "a"), _dev_ptr(X, "X"), _dev_ptr(Y, "Y"),
+                                              _dev_ptr(K, "K")), "bkr_block_axpy_gram")
+        return K
 
     def cholesky_upper(self, H):
         N = int(H.shape[0])

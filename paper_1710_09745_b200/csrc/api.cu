@@ -115,6 +115,14 @@ int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, 
     return launch_block_update(ctx, N, prec, prec, (const double2 *)a, Y, X, Y, nullptr);
 }
 
+int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y, void *K)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !a || !X || !Y || !K || X == Y) return BKR_EINVAL;
+    int np = 0;
+    BKR_TRY(launch_update_gram(ctx, N, prec, (const double2 *)a, Y, X, Y, &np, nullptr));
+    return launch_gram_finish(ctx, N, np, 1, (double2 *)K);
+}
+
 int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, int *status)
 {
     if (!ctx || !valid_n(N) || !H || !R) return BKR_EINVAL;

@@ -185,6 +185,41 @@ def test_block_axpy_fp32(lat_asym, N):
     assert H.relerr_inf(got, oracle.block_axpy(a, X, Y)) <= TOL32
 
 
+@pytest.mark.parametrize("N", [1, 3, 8, 13, 16, 24, 32])
+def test_block_axpy_gram_fused_fp64(lat_asym, N):
+    """fused update + aliased Hermitian Gram (Alg. 1 l.11 + Alg. 2 l.2) against the oracle's two separate operations"""
+    dims, _, _, ctx = lat_asym
+    X, Y = H.np_sources(dims, N, 1400 + N), H.np_sources(dims, N, 1500 + N)
+    rng = np.random.default_rng(100 + N)
+    a = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    Xd, Yd = ctx.pack(torch.from_numpy(X).cuda()), ctx.pack(torch.from_numpy(Y).cuda())
+    K = ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd).cpu().numpy()
+    want = oracle.block_axpy(a, X, Y)
+    assert H.relerr_inf(ctx.unpack(Yd, N).cpu().numpy(), want) <= TOL64
+    wantK = oracle.gram(want, want)
+    assert np.abs(K - wantK).max() <= 1e-13 * np.abs(wantK).max()
+    assert np.array_equal(K, K.conj().T) and np.all(K.diagonal().imag == 0)
+    # P12: bit-identical on repetition from the same inputs
+    Yd2 = ctx.pack(torch.from_numpy(Y).cuda())
+    assert torch.equal(ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd2).cpu(), torch.from_numpy(K))
+
+
+@pytest.mark.parametrize("N", [4, 16])
+def test_block_axpy_gram_fused_fp32(lat_asym, N):
+    """fp32 blocks: K is the fp64-accumulated Gram matrix of the fp32-rounded result"""
+    from paper_1710_09745_b200 import binding
+    dims, _, _, ctx = lat_asym
+    X, Y = _round32(H.np_sources(dims, N, 1600 + N)), _round32(H.np_sources(dims, N, 1700 + N))
+    rng = np.random.default_rng(200 + N)
+    a = _round32(rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N)))
+    Xd, Yd = ctx.pack(torch.from_numpy(X).cuda(), binding.F32), ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
+    K = ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd, prec=binding.F32).cpu().numpy()
+    got = ctx.unpack(Yd, N, binding.F32).cpu().numpy()
+    assert H.relerr_inf(got, oracle.block_axpy(a, X, Y)) <= TOL32
+    wantK = oracle.gram(got, got)  # of the stored (rounded) block: fp64 products of fp32 numbers are exact
+    assert np.abs(K - wantK).max() <= 1e-13 * np.abs(wantK).max()
+
+
 @pytest.mark.parametrize("N", [1, 2, 5, 8, 16, 32])
 def test_small_matrix_kernel(lat4, N):
     """pin P11 through the CUDA path: Cholesky / triangular inverse / HPD inverse vs the oracle."""
