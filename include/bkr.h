@@ -111,6 +111,15 @@ int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, 
  * with a real diagonal, bit-reproducible.  a, K: N*N complex fp64 (device); X, Y native, X != Y. */
 int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y, void *K);
 
+/* The fused update the solver runs at the top of an iteration (Algorithm 2 l.4 of the previous iteration, Algorithm 1
+ * l.8, and the deferred l.10 of the previous iteration), one pass over Q, P, X:
+ *     if do_qp:  Q <- Q Sinv (in place);  Pn <- Q + P Sdag        Sinv UPPER triangular, Sdag LOWER triangular:
+ *     if do_x :  X <- X + P Wm (in place)                          entries on the other side are NOT read
+ * Sinv, Sdag, Wm: N*N complex fp64 (device).  Q, P, Pn: native blocks of precision prec, Pn != P; X: native fp64 block
+ * (also when prec is fp32).  N <= 24 is what the solver uses it for; any 1 <= N <= 32 is accepted. */
+int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const void *Sdag, const void *Wm, void *Q,
+                         const void *P, void *Pn, void *X, int do_qp, int do_x);
+
 /* Small dense algebra on the device, one warp (Algorithm 2 l.3):
  * bkr_cholesky_upper: H = R^dag R, R upper triangular with real positive diagonal; Rinv = R^-1.
  * bkr_hpd_inverse   : Ginv = G^-1 for Hermitian positive-definite G (via Cholesky).

@@ -19,7 +19,7 @@ MAX_N = 32
 
 SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash",
-    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_axpy_gram", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
+    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
     "bkr_strerror", "bkr_version", "bkr_dslash_variant",
 )
@@ -66,6 +66,7 @@ def lib():
             "bkr_gram": (ci, [vp, ci, ci, vp, vp, ci, vp]),
             "bkr_block_axpy": (ci, [vp, ci, ci, vp, vp, vp]),
             "bkr_block_axpy_gram": (ci, [vp, ci, ci, vp, vp, vp, vp]),
+            "bkr_block_qpx_update": (ci, [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, ci, ci]),
             "bkr_cholesky_upper": (ci, [vp, ci, vp, vp, vp, vp]),
             "bkr_hpd_inverse": (ci, [vp, ci, vp, vp, vp]),
             "bkr_solve_block": (ci, [vp, cd, ci, vp, vp, cd, ci, ci, cd, vp, ctypes.POINTER(Stats)]),
@@ -193,6 +194,14 @@ class Context:
         self._check(lib().bkr_block_axpy_gram(self._h, int(N), int(prec), _dev_ptr(a, "a"), _dev_ptr(X, "X"), _dev_ptr(Y, "Y"),
                                               _dev_ptr(K, "K")), "bkr_block_axpy_gram")
         return K
+
+    def block_qpx_update(self, N, Sinv, Sdag, Wm, Q, P, Pn, X, prec=F64, do_qp=True, do_x=True):
+        """Q <- Q Sinv, Pn <- Q + P Sdag (if do_qp) and X <- X + P Wm (if do_x) in one pass (bkr.h)."""
+        for m in (Sinv, Sdag, Wm):
+            assert m.dtype == torch.complex128 and tuple(m.shape) == (int(N), int(N))
+        self._check(lib().bkr_block_qpx_update(self._h, int(N), int(prec), _dev_ptr(Sinv, "Sinv"), _dev_ptr(Sdag, "Sdag"),
+                                               _dev_ptr(Wm, "Wm"), _dev_ptr(Q, "Q"), _dev_ptr(P, "P"), _dev_ptr(Pn, "Pn"),
+                                               _dev_ptr(X, "X"), int(bool(do_qp)), int(bool(do_x))), "bkr_block_qpx_update")
 
     def cholesky_upper(self, H):
         N = int(H.shape[0])

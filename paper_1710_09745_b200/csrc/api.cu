@@ -49,6 +49,7 @@ int bkr_destroy(bkr_ctx *ctx)
     cudaFree(ctx->links32);
     cudaFree(ctx->tile_order);
     cudaFree(ctx->win_segs);
+    cudaFree(ctx->api_flags);
     cudaFree(ctx->tmp_odd[0]);
     cudaFree(ctx->tmp_odd[1]);
     cudaFree(ctx->partials);
@@ -121,6 +122,23 @@ int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void
     int np = 0;
     BKR_TRY(launch_update_gram(ctx, N, prec, (const double2 *)a, Y, X, Y, &np, nullptr));
     return launch_gram_finish(ctx, N, np, 1, (double2 *)K);
+}
+
+int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const void *Sdag, const void *Wm, void *Q,
+                         const void *P, void *Pn, void *X, int do_qp, int do_x)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !Sinv || !Sdag || !Wm || !Q || !P || !Pn || !X || P == Pn) return BKR_EINVAL;
+    if (!ctx->api_flags) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->api_flags, sizeof(SolverFlags)));
+    SolverFlags f;
+    memset(&f, 0, sizeof(f));
+    f.done = do_qp ? 0 : 1;
+    f.xpend = do_x ? 1 : 0;
+    f.xidle = do_x ? 0 : 1;
+    // small synchronous copy from the stack: ordered before the kernel by the stream synchronisation
+    BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    BKR_CUDA(ctx, cudaMemcpy(ctx->api_flags, &f, sizeof(f), cudaMemcpyHostToDevice));
+    return launch_pqx_update(ctx, N, prec, (const double2 *)Sinv, (const double2 *)Sdag, (const double2 *)Wm, Q, P, Pn,
+                             (double2 *)X, ctx->api_flags);
 }
 
 int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, int *status)

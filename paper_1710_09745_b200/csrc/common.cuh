@@ -60,6 +60,7 @@ struct bkr_ctx {
     // segment table of the window stencil (dslash_win.cu): (first tile, end tile, strip first, strip last)
     int4 *win_segs;
     int win_nseg, win_key;
+    SolverFlags *api_flags; // device flags for the API-level fused update
     int dslash_nblock;  // rhs count of the whole block while launch_dslash works through it in chunks (L2 blocking uses it)
     int dslash_variant; // last stencil kernel used: 0 plain, 1 window, -1 none yet
     // scratch for apply_M (odd-parity temporary), grown on demand, per precision

@@ -204,6 +204,46 @@ def test_block_axpy_gram_fused_fp64(lat_asym, N):
     assert torch.equal(ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd2).cpu(), torch.from_numpy(K))
 
 
+@pytest.mark.parametrize("N", [1, 4, 7, 13, 16, 24, 32])
+def test_block_qpx_update_fp64(lat_asym, N):
+    """fused Q / P / X update with triangular coefficients against three oracle block updates; the
+    entries on the wrong side of Sinv / Sdag are poisoned to prove they are never read"""
+    dims, _, _, ctx = lat_asym
+    Q, P, X = (H.np_sources(dims, N, 1800 + 10 * k + N) for k in range(3))
+    rng = np.random.default_rng(300 + N)
+    full = lambda: rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    Sinv, Sdag, Wm = np.triu(full()), np.tril(full()), full()
+    poison = 1e30
+    Sinv_d = torch.from_numpy(Sinv + poison * np.tril(np.ones((N, N)), -1) * _frag_mask(N, upper=True)).cuda()
+    Sdag_d = torch.from_numpy(Sdag + poison * np.triu(np.ones((N, N)), 1) * _frag_mask(N, upper=False)).cuda()
+    Qd, Pd, Xd = (ctx.pack(torch.from_numpy(v).cuda()) for v in (Q, P, X))
+    Pn = torch.empty_like(Pd)
+    ctx.block_qpx_update(N, Sinv_d, Sdag_d, torch.from_numpy(Wm).cuda(), Qd, Pd, Pn, Xd)
+    Qn = oracle.block_axpy(Sinv, Q, np.zeros_like(Q))
+    assert H.relerr_inf(ctx.unpack(Qd, N).cpu().numpy(), Qn) <= TOL64
+    assert H.relerr_inf(ctx.unpack(Pn, N).cpu().numpy(), oracle.block_axpy(Sdag, P, Qn)) <= TOL64
+    assert H.relerr_inf(ctx.unpack(Xd, N).cpu().numpy(), oracle.block_axpy(Wm, P, X)) <= TOL64
+    # gating: do_x only leaves Q untouched
+    Qd2, Xd2 = ctx.pack(torch.from_numpy(Q).cuda()), ctx.pack(torch.from_numpy(X).cuda())
+    ctx.block_qpx_update(N, Sinv_d, Sdag_d, torch.from_numpy(Wm).cuda(), Qd2, Pd, Pn, Xd2, do_qp=False, do_x=True)
+    assert torch.equal(Qd2, ctx.pack(torch.from_numpy(Q).cuda()))
+    assert H.relerr_inf(ctx.unpack(Xd2, N).cpu().numpy(), oracle.block_axpy(Wm, P, X)) <= TOL64
+
+
+def _frag_mask(N, upper):
+    """1 where a whole 4 x 8 DMMA coefficient fragment lies strictly on the zero side of the triangle (those fragments
+    are skipped); entries of fragments that straddle the diagonal are read and must be true zeros"""
+    m = np.zeros((N, N))
+    for i in range(N):
+        for j in range(N):
+            i0, j0 = 4 * (i // 4), 8 * (j // 8)
+            if upper and i0 > j0 + 7:
+                m[i, j] = 1.0
+            if not upper and i0 + 3 < j0:
+                m[i, j] = 1.0
+    return m
+
+
 @pytest.mark.parametrize("N", [4, 16])
 def test_block_axpy_gram_fused_fp32(lat_asym, N):
     """fp32 blocks: K is the fp64-accumulated Gram matrix of the fp32-rounded result"""
