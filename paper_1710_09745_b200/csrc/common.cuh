@@ -128,8 +128,9 @@ int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const voi
 int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K);
 // Z = C + W a   (C may be NULL = 0; Z may alias C; Z must not alias W).  a: N x N complex fp64 (device).
 // precZ is the precision of Z and C, precW of W; arithmetic in precZ.
+// tri: 0 = general a, 1 = a upper triangular, 2 = a lower triangular (entries on the other side are not read).
 int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C,
-                        const void *W, void *Z, const int *done);
+                        const void *W, void *Z, const int *done, int tri = 0);
 // Deferred X update fused with the P update (Alg. 1 l.10 of the previous iteration + l.8 of this one):
 //   if (flags->xpend)  X  += P Wm          (X fp64, in place)
 //   if (!flags->done)  Pn  = Q + P Sdag    (Pn must not alias P)

@@ -122,7 +122,7 @@ static RingPlan plan_ring(size_t L, size_t fixed, int min_stages, int nchunk_a, 
 template <typename RealZ, typename RealW, int NTJ, int NIS, bool HASC, int CW>
 __global__ void __launch_bounds__((CW + 1) * 32, 1)
 update_tma_kernel(size_t L, int N, RingPlan rp, const double2 *__restrict__ a, const typename CxT<RealZ>::type *C,
-                  const typename CxT<RealW>::type *__restrict__ W, typename CxT<RealZ>::type *Z, const int *done)
+                  const typename CxT<RealW>::type *__restrict__ W, typename CxT<RealZ>::type *Z, const int *done, int tri)
 {
     typedef typename CxT<RealZ>::type CxZ;
     typedef typename CxT<RealW>::type CxW;
@@ -208,6 +208,8 @@ update_tma_kernel(size_t L, int N, RingPlan rp, const double2 *__restrict__ a, c
             for (int is = 0; is < NIS; is++) {
 #pragma unroll
                 for (int tj = 0; tj < NTJ; tj++) {
+                    // triangular coefficients: fragments wholly on the zero side are skipped, not read
+                    if ((tri == 1 && 4 * is > 8 * tj + 7) || (tri == 2 && 4 * is + 3 < 8 * tj)) continue;
                     const int f = is * NTJ + tj;
                     const double br = BREG ? ar[f] : bre[f * 32 + lane], bi = BREG ? ai[f] : bim[f * 32 + lane];
                     dmma(zre[tj], wf[is].x, br);
@@ -239,7 +241,7 @@ update_tma_kernel(size_t L, int N, RingPlan rp, const double2 *__restrict__ a, c
 }
 
 template <typename RealZ, typename RealW, int NTJ, int NIS>
-static int update_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done)
+static int update_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done, int tri)
 {
     typedef typename CxT<RealZ>::type CxZ;
     typedef typename CxT<RealW>::type CxW;
@@ -259,19 +261,19 @@ static int update_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const void
     }
     if (C)
         update_tma_kernel<RealZ, RealW, NTJ, NIS, true, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
-            L, N, rp, a, (const CxZ *)C, (const CxW *)W, (CxZ *)Z, done);
+            L, N, rp, a, (const CxZ *)C, (const CxW *)W, (CxZ *)Z, done, tri);
     else
         update_tma_kernel<RealZ, RealW, NTJ, NIS, false, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
-            L, N, rp, a, nullptr, (const CxW *)W, (CxZ *)Z, done);
+            L, N, rp, a, nullptr, (const CxW *)W, (CxZ *)Z, done, tri);
     return bkr_check_launch(ctx);
 }
 
 template <typename RealZ, typename RealW>
-static int launch_update_t(bkr_ctx *ctx, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done)
+static int launch_update_t(bkr_ctx *ctx, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done, int tri)
 {
     const size_t L = (size_t)ctx->g.Vh * 3;
     const int NIS = (N + 3) / 4;
-#define UPD_GO(NTJ_, NIS_) return update_go<RealZ, RealW, NTJ_, NIS_>(ctx, L, N, a, C, W, Z, done)
+#define UPD_GO(NTJ_, NIS_) return update_go<RealZ, RealW, NTJ_, NIS_>(ctx, L, N, a, C, W, Z, done, tri)
     switch (NIS) {
     case 1: UPD_GO(1, 1);
     case 2: UPD_GO(1, 2);
@@ -286,13 +288,13 @@ static int launch_update_t(bkr_ctx *ctx, int N, const double2 *a, const void *C,
 }
 
 int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C, const void *W, void *Z,
-                        const int *done)
+                        const int *done, int tri)
 {
-    if (precZ == BKR_F64 && precW == BKR_F64) return launch_update_t<double, double>(ctx, N, a, C, W, Z, done);
-    if (precZ == BKR_F64 && precW == BKR_F32) return launch_update_t<double, float>(ctx, N, a, C, W, Z, done);
-    if (precZ == BKR_F32 && precW == BKR_F32) return launch_update_t<float, float>(ctx, N, a, C, W, Z, done);
+    if (precZ == BKR_F64 && precW == BKR_F64) return launch_update_t<double, double>(ctx, N, a, C, W, Z, done, tri);
+    if (precZ == BKR_F64 && precW == BKR_F32) return launch_update_t<double, float>(ctx, N, a, C, W, Z, done, tri);
+    if (precZ == BKR_F32 && precW == BKR_F32) return launch_update_t<float, float>(ctx, N, a, C, W, Z, done, tri);
     // fp32 <- fp64: only Qhat = R C^-1 of the reliable update (Alg. 3 l.5), computed in fp64, rounded on store
-    return launch_update_t<float, double>(ctx, N, a, C, W, Z, done);
+    return launch_update_t<float, double>(ctx, N, a, C, W, Z, done, tri);
 }
 
 // ------------------------------------------------------------------------------------------ Gram, stage 1

@@ -171,7 +171,7 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
     BKR_TRY(launch_gram_partials(ctx, N, BKR_F64, w->R64, w->R64, 1, &np, gate));
     BKR_TRY(launch_small(ctx, small_args(w, small_mode, np, tol, delta, mixed, ctx)));
     // Q = R C^-1 (Alg. 2 l.4), stored in the inner precision
-    BKR_TRY(launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr));
+    BKR_TRY(launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr, 1)); // C^-1 upper triangular
     if (fuse_q(N)) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
         set_identity_kernel<<<1, 256, 0, ctx->stream>>>(N, w->Sinv);
         BKR_TRY(bkr_check_launch(ctx));
@@ -220,7 +220,7 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
         if (fuse_q(N)) BKR_TRY(launch_pqx_update(ctx, N, pr, w->Sinv, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
         else BKR_TRY(launch_px_update(ctx, N, pr, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
     } else {
-        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done));
+        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done, 2)); // S^dag lower triangular
     }
     t = w->P; w->P = w->P2; w->P2 = t;
     // l.9  beta = (P^dag M P)^-1 ; W = beta C
@@ -242,7 +242,7 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     // l.12 C = S C, residual norms, convergence / reliable-update flags
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_QR, np, tol, delta, mixed, ctx)));
     if (!fuse_q(N)) {
-        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done));
+        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done, 1)); // S^-1 upper triangular
         t = w->Q; w->Q = w->Q2; w->Q2 = t;
     }
     return BKR_OK;
