@@ -137,7 +137,8 @@ template <typename Real, typename Cx> __device__ __forceinline__ void cfma3(Real
 }
 
 // blockDim = (4 G + 4) warps: warps [0, 2G) = set A (x/y hops), [2G, 4G) = set B (z/t hops), last 4 warps = producers.
-// Inside a set, warp w handles rhs group w / 2 (T rhs) and sites (w % 2) * 32 + lane of the 64-site tile.
+// Inside a set, warp w handles sites (w % 4) * 16 + lane % 16 of the 64-site tile and the rhs groups 2 (w / 4) + lane / 16
+// (T rhs each); for odd G: rhs group w / 2 and sites (w % 2) * 32 + lane.
 template <typename Real, int T, int G, int C, bool XP>
 __global__ void __launch_bounds__((4 * G + 4) * 32, 1)
 dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_constant__ CUtensorMap tm_zt,
@@ -281,7 +282,10 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
         // ------------------------------------------------------------------ set A: x/y hops from the window
         // The window is cyclic in y: virtual chunk c of a strip is memory chunk cs + (c - cs) mod ncs, so the wrapped
         // neighbours of the first and last rows of a strip are served like all others (no global loads here at all).
-        const int sl = (warp & 1) * 32 + lane, j0 = (warp >> 1) * T;
+        // lanes 0-15 and 16-31 of a warp: the same 16 sites, two rhs groups -- the link loads of the two half-warps hit the
+        // same shared-memory addresses (one broadcast wavefront pair instead of two): half the link traffic on the port
+        const int sl = (G % 2 == 0) ? (warp & 3) * 16 + (lane & 15) : (warp & 1) * 32 + lane;
+        const int j0 = (G % 2 == 0) ? (2 * (warp >> 2) + (lane >> 4)) * T : (warp >> 1) * T;
         int tc = 0, q0 = 0;
         for (int si = cid; si < p.nseg; si += ncl) {
             const int4 sg = p.segs[si];
@@ -389,7 +393,8 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
         // ------------------------------------------------------------------ set B: z/t hops from the sub-stage ring,
         // then the epilogue: add set A's partial sums, out = acc  or  a * xp - acc
         const int wb = warp - NWS;
-        const int sl = (wb & 1) * 32 + lane, j0 = (wb >> 1) * T;
+        const int sl = (G % 2 == 0) ? (wb & 3) * 16 + (lane & 15) : (wb & 1) * 32 + lane;
+        const int j0 = (G % 2 == 0) ? (2 * (wb >> 2) + (lane >> 4)) * T : (wb >> 1) * T;
         const int jg = (int)rank * NC + j0; // first global rhs of this thread
         int tc = 0;
         for (int si = cid; si < p.nseg; si += ncl) {
