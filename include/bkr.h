@@ -158,10 +158,30 @@ int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void 
                          long long *launches);
 
 /* Which stencil kernel the most recent Dslash launch of this context used (bkr_dslash, bkr_apply_M or inside a solver):
- * 0 = plain multi-rhs kernel (register tiling + link ring), 1 = shared-memory window kernel with
+ * 0 = plain multi-rhs kernel (register tiling + link ring), 2 = row-window kernel, 1 = shared-memory window kernel with
  * cluster-multicast links (same operation; chosen per lattice/N/precision),
  * -1 = none yet.  Diagnostic only. */
 int bkr_dslash_variant(const bkr_ctx *ctx);
+
+/* Force the stencil kernel of later calls (tests and measurements; every variant computes the same operation):
+ * -1 = automatic choice (default), 0 = plain kernel, 1 = window kernel, 2 = row-window kernel (16 rhs per CTA, z/t
+ * neighbours by register loads; fp64, X = 32).  A forced variant that cannot run the lattice / N falls back to the
+ * plain kernel; bkr_dslash_variant() tells which one ran. */
+int bkr_set_dslash_variant(bkr_ctx *ctx, int variant);
+
+/* Launch-policy knobs (the paper's autotuner picks such parameters on first call; here they have measured
+ * defaults and this call overrides them for sweeps).  value 0 restores the default.
+ *   BKR_OPT_L2_BUDGET_MB    L2 working-set budget (MB) that sizes the z blocks of the stencil's sweep order
+ *   BKR_OPT_ROW_UNIT_TILES  64-site tiles per work unit of the row-window stencil (1, 2, 4, 8 ...)
+ *   BKR_OPT_ROW_VEC_POLICY  L2 eviction priority of its z/t neighbour loads: 0 normal, 1 evict_last, 2 evict_first */
+enum { BKR_OPT_L2_BUDGET_MB = 0, BKR_OPT_ROW_UNIT_TILES = 1, BKR_OPT_ROW_VEC_POLICY = 2 };
+int bkr_set_option(bkr_ctx *ctx, int option, int value);
+
+/* Measured on-chip peaks for the rooflines (not on the hot path).  kind: 0 fp64 FMA, 1 fp32 FMA,
+ * 2 fp64 tensor MMA (m8n8k4), 3 L2 -> SM bandwidth by 16-byte loads, 4 the same by TMA bulk copies, 5 shared-memory read
+ * bandwidth.  Runs `reps` launches on the context's stream, synchronises, and writes result[0] = ms per launch,
+ * result[1] = flop (kinds 0-2) or bytes (kinds 3-5) per launch.  result: HOST array of 2 doubles. */
+int bkr_microbench(bkr_ctx *ctx, int kind, int reps, double *result);
 
 int bkr_last_cuda_error(const bkr_ctx *ctx);
 const char *bkr_strerror(int status);

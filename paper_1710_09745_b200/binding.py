@@ -16,12 +16,13 @@ LIB_PATH = os.path.join(_HERE, "libbkr.so")
 F64, F32 = 0, 1
 OK, EINVAL, ENOLINKS, ENOMEM, ECUDA, EBREAKDOWN, ENOCONV = 0, -1, -2, -3, -4, -5, -6
 MAX_N = 32
+OPT_L2_BUDGET_MB, OPT_ROW_UNIT_TILES = 0, 1
 
 SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash",
     "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
-    "bkr_strerror", "bkr_version", "bkr_dslash_variant",
+    "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench",
 )
 
 
@@ -78,6 +79,9 @@ def lib():
             "bkr_strerror": (ctypes.c_char_p, [ci]),
             "bkr_version": (ctypes.c_char_p, []),
             "bkr_dslash_variant": (ci, [vp]),
+            "bkr_set_dslash_variant": (ci, [vp, ci]),
+            "bkr_set_option": (ci, [vp, ci, ci]),
+            "bkr_microbench": (ci, [vp, ci, ci, ctypes.POINTER(cd)]),
         }
         for name, (res, args) in sig.items():
             f = getattr(L, name)
@@ -287,8 +291,22 @@ class Context:
                                                ctypes.byref(n)), "bkr_bench_iterations")
         return int(n.value)
 
+    def microbench(self, kind, reps=5):
+        """(ms per launch, flop or bytes per launch) of the on-chip microbenchmark `kind` (bkr.h)."""
+        r = (ctypes.c_double * 2)()
+        self._check(lib().bkr_microbench(self._h, int(kind), int(reps), r), "bkr_microbench")
+        return float(r[0]), float(r[1])
+
+    def set_option(self, option, value):
+        """launch-policy knob (bkr.h BKR_OPT_*): OPT_L2_BUDGET_MB = 0, OPT_ROW_UNIT_TILES = 1; value 0 = default."""
+        self._check(lib().bkr_set_option(self._h, int(option), int(value)), "bkr_set_option")
+
+    def set_dslash_variant(self, variant):
+        """-1 automatic, 0 plain, 1 window, 2 row-window stencil kernel for later calls (bkr.h)."""
+        self._check(lib().bkr_set_dslash_variant(self._h, int(variant)), "bkr_set_dslash_variant")
+
     def dslash_variant(self):
-        """0 = plain stencil kernel, 1 = shared-memory window kernel, -1 = no Dslash launched yet (diagnostic)."""
+        """0 = plain stencil kernel, 1 = shared-memory window kernel, 2 = row-window kernel, -1 = none yet (diagnostic)."""
         return int(lib().bkr_dslash_variant(self._h))
 
 

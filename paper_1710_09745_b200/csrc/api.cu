@@ -30,6 +30,7 @@ int bkr_create(bkr_ctx **out, const int dims[4], int device, void *cuda_stream)
     ctx->g.Vh = (int)(V / 2);
     ctx->device = device;
     ctx->dslash_variant = -1;
+    ctx->dslash_force = -1;
     ctx->stream = (cudaStream_t)cuda_stream;
     if (cudaMalloc((void **)&ctx->small, (size_t)4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)) != cudaSuccess) {
         free(ctx);
@@ -49,6 +50,7 @@ int bkr_destroy(bkr_ctx *ctx)
     cudaFree(ctx->links32);
     cudaFree(ctx->tile_order);
     cudaFree(ctx->win_segs);
+    cudaFree(ctx->row_strips);
     cudaFree(ctx->api_flags);
     cudaFree(ctx->tmp_odd[0]);
     cudaFree(ctx->tmp_odd[1]);
@@ -253,6 +255,12 @@ int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void 
     return solver_bench_iterations(ctx, mass, N, prec, (const double2 *)B, iters, launches);
 }
 
+int bkr_microbench(bkr_ctx *ctx, int kind, int reps, double *result)
+{
+    if (!ctx) return BKR_EINVAL;
+    return run_microbench(ctx, kind, reps, result);
+}
+
 int bkr_last_cuda_error(const bkr_ctx *ctx) { return ctx ? ctx->last_cuda : 0; }
 
 const char *bkr_strerror(int status)
@@ -270,6 +278,27 @@ const char *bkr_strerror(int status)
 }
 
 int bkr_dslash_variant(const bkr_ctx *ctx) { return ctx ? ctx->dslash_variant : -1; }
+
+int bkr_set_option(bkr_ctx *ctx, int option, int value)
+{
+    if (!ctx || value < 0) return BKR_EINVAL;
+    switch (option) {
+    case BKR_OPT_L2_BUDGET_MB: ctx->l2_budget_mb = value; break;
+    case BKR_OPT_ROW_UNIT_TILES: ctx->row_unit_tiles = value; break;
+    case BKR_OPT_ROW_VEC_POLICY: ctx->row_vec_policy = value; break;
+    default: return BKR_EINVAL;
+    }
+    // blocking tables are rebuilt on the next stencil call
+    ctx->tile_order_key = ctx->win_key = ctx->row_key = -1;
+    return BKR_OK;
+}
+
+int bkr_set_dslash_variant(bkr_ctx *ctx, int variant)
+{
+    if (!ctx || variant < -1 || variant > 2) return BKR_EINVAL;
+    ctx->dslash_force = variant;
+    return BKR_OK;
+}
 
 const char *bkr_version(void) { return "libbkr 0.1 (sm_100a)"; }
 

@@ -60,6 +60,11 @@ struct bkr_ctx {
     // segment table of the window stencil (dslash_win.cu): (first tile, end tile, strip first, strip last)
     int4 *win_segs;
     int win_nseg, win_key;
+    // strip table of the row-window stencil (dslash_row.cu): first tile of each (z, t) strip in processing order
+    int *row_strips;
+    int row_nstrip, row_key;
+    int dslash_force; // bkr_set_dslash_variant: -1 automatic, 0 plain, 1 window, 2 row window
+    int l2_budget_mb, row_unit_tiles, row_vec_policy; // bkr_set_option (0 = built-in default)
     SolverFlags *api_flags; // device flags for the API-level fused update
     int dslash_nblock;  // rhs count of the whole block while launch_dslash works through it in chunks (L2 blocking uses it)
     int dslash_variant; // last stencil kernel used: 0 plain, 1 window, -1 none yet
@@ -118,6 +123,10 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
 
 // ---- dslash_win.cu : same operation, shared-memory window version; returns 1 when not applicable
 int launch_dslash_win(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp,
+                      double a, const int *done);
+
+// ---- dslash_row.cu : same operation, row-window version for 9..32 fp64 rhs; returns 1 when not applicable
+int launch_dslash_row(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp,
                       double a, const int *done);
 
 // ---- blas.cu
@@ -182,6 +191,9 @@ struct CgScalars {
     int iters[BKR_MAX_N], conv[BKR_MAX_N];
 };
 int launch_cg_scalar(bkr_ctx *ctx, int N, int step, double tol, CgScalars *s, SolverFlags *flags);
+
+// ---- microbench.cu
+int run_microbench(bkr_ctx *ctx, int kind, int reps, double *result);
 
 // ---- solver.cu
 int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, double tol, int maxiter,

@@ -206,8 +206,7 @@ static int build_tile_order(bkr_ctx *ctx, int N, int prec)
 {
     const Geom &g = ctx->g;
     const int Xh = g.X[0] / 2, Y = g.X[1], Z = g.X[2], Tt = g.X[3];
-    static const char *env = getenv("BKR_L2_BUDGET_MB");
-    const double budget = (env ? atof(env) : 48.0) * 1e6;
+    const double budget = (ctx->l2_budget_mb > 0 ? ctx->l2_budget_mb : 48) * 1e6;
     const double site_bytes = 3.0 * std::max(N, ctx->dslash_nblock) * (prec == BKR_F64 ? 16 : 8);
     int bestY = Y, bestZ = Z;
     double best_cost = 1e30, best_ws = 0;
@@ -348,12 +347,20 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
                   const int *done)
 {
     if (!(prec == BKR_F64 ? (void *)ctx->links64 : (void *)ctx->links32)) return BKR_ENOLINKS;
-    // fp64 blocks of more than 16 rhs go through in chunks of 16: two cluster-of-2 window launches beat one cluster of 4
-    // (32^3 x 64, N = 32: 2 x 1.32 ms against 3.02 ms; 48^3 x 96: 2 x 7.3 ms against 19.1 ms for the plain kernel) although
+    // the row-window kernel takes whole fp64 blocks of 9..32 rhs on X = 32 lattices, every link read once (dslash_row.cu)
+    if (!ctx->dslash_nblock) {
+        const int rc = launch_dslash_row(ctx, out_parity, N, prec, in, out, xp, a, done);
+        if (rc != 1) {
+            ctx->dslash_variant = 2;
+            return rc;
+        }
+    }
+    // Elsewhere fp64 blocks of more than 16 rhs go through in chunks of 16: two cluster-of-2 window launches beat one cluster
+    // of 4 (32^3 x 64, N = 32: 2 x 1.32 ms against 3.02 ms; 48^3 x 96: 2 x 7.3 ms against 19.1 ms for the plain kernel) although
     // the links are then read once per chunk.  A chunk is a contiguous view of the native block [rhs][colour][site].
     // Likewise 11-13 rhs as 8 + rest (window kernel + plain kernel) and fp32 blocks of 17-28 rhs as 16 + rest.
     int chunk = 0;
-    if (!getenv("BKR_DSLASH_NOSPLIT")) {
+    if (ctx->dslash_force < 0 || ctx->dslash_force == 1) {
         if (prec == BKR_F64 && N > 16) chunk = 16;
         else if (prec == BKR_F64 && N >= 11 && N <= 13) chunk = 8; // 14 = window cluster of 2 (1.29 ms) beats 8 + 6 (1.32 ms)
         else if (prec == BKR_F32 && N > 16 && N <= 28) chunk = 16;
@@ -370,7 +377,7 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
         ctx->dslash_nblock = 0;
         return rc;
     }
-    {
+    if (ctx->dslash_force != 0 && ctx->dslash_force != 2) {
         const int rc = launch_dslash_win(ctx, out_parity, N, prec, in, out, xp, a, done);
         if (rc != 1) {
             ctx->dslash_variant = 1;

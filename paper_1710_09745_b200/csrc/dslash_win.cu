@@ -519,8 +519,7 @@ static int build_segments(bkr_ctx *ctx, int N, int prec, int seglen)
 {
     const Geom &g = ctx->g;
     const int Xh = g.X[0] / 2, Y = g.X[1], Z = g.X[2], Tt = g.X[3];
-    static const char *env = getenv("BKR_L2_BUDGET_MB");
-    const double budget = (env ? atof(env) : 48.0) * 1e6;
+    const double budget = (ctx->l2_budget_mb > 0 ? ctx->l2_budget_mb : 48) * 1e6;
     const double site_bytes = 3.0 * std::max(N, ctx->dslash_nblock) * (prec == BKR_F64 ? 16 : 8);
     int zb = 1;
     for (int c = 1; c <= Z; c++)
@@ -584,8 +583,7 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     {
         // clusters of 3-4 CTAs need the deep link ring (the release -> refill round trip crosses SMs): with 4 stages the
         // plain kernel is faster (48^3 x 96, N = 32 fp64: 20.6 vs 19.1 ms), with 8 it is not (32^3 x 64: 3.02 vs 3.10 ms)
-        const char *menv = getenv("BKR_DSLASH_WIN");
-        if (C >= 3 && rl < 8 && !(menv && atoi(menv) == 2)) return 1;
+        if (C >= 3 && rl < 8 && ctx->dslash_force != 1) return 1;
     }
     if (nz < 2 && !getenv("BKR_WIN_ALLOW_NZ1")) return 1; // one z/t stage: slower than dslash.cu (48^4: 2.6 vs 2.1 ms)
     p.nzlog = nz == 4 ? 2 : nz == 2 ? 1 : 0;
@@ -669,8 +667,7 @@ static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *i
 int launch_dslash_win(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp, double a,
                       const int *done)
 {
-    const char *menv = getenv("BKR_DSLASH_WIN"); // 0: never, 1: automatic (default), 2: whenever the geometry allows
-    const int mode = menv ? atoi(menv) : 1;
+    const int mode = ctx->dslash_force == 1 ? 2 : 1; // 1: automatic, 2: whenever the geometry allows (bkr_set_dslash_variant)
     const Geom &g = ctx->g;
     const int Xh = g.X[0] / 2;
     if (mode == 0 || (Xh * g.X[1]) % 64 != 0) return 1;
