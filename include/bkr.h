@@ -105,6 +105,13 @@ int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int he
  * streamed once.  a: N*N complex fp64; X, Y native, X != Y. */
 int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y);
 
+/* The general form the solver uses (eq. 3; "templated on ... Y precision >= X precision", PAPER.md:260;
+ * triangular coefficient matrices in Algorithm 1 l.8 and Algorithm 2 l.4):   Z <- C + W a.
+ * Z, C: native blocks of precision precZ (C may be NULL = 0; Z may alias C); W: native block of precision precW, W != Z;
+ * arithmetic and accumulation in fp64, rounded to precZ on store.  tri: 0 = general a, 1 = a upper triangular, 2 = a lower
+ * triangular: the entries on the zero side are NOT read (they may hold anything). */
+int bkr_block_update(bkr_ctx *ctx, int N, int precZ, int precW, int tri, const void *a, const void *C, const void *W, void *Z);
+
 /* The two fused, as the solver uses them for Algorithm 1 l.11 + Algorithm 2 l.2 (aliased
  * Hermitian reduction PAPER.md:289):  Y <- Y + X a  and  K = Y^dag Y  of the updated Y, in one pass over X and Y.
  * K is the Gram matrix of Y as stored (for fp32 blocks: of the fp32-rounded result), accumulated in fp64, Hermitian
@@ -173,8 +180,17 @@ int bkr_set_dslash_variant(bkr_ctx *ctx, int variant);
  * defaults and this call overrides them for sweeps).  value 0 restores the default.
  *   BKR_OPT_L2_BUDGET_MB    L2 working-set budget (MB) that sizes the z blocks of the stencil's sweep order
  *   BKR_OPT_ROW_UNIT_TILES  64-site tiles per work unit of the row-window stencil (1, 2, 4, 8 ...)
- *   BKR_OPT_ROW_VEC_POLICY  L2 eviction priority of its z/t neighbour loads: 0 normal, 1 evict_last, 2 evict_first */
-enum { BKR_OPT_L2_BUDGET_MB = 0, BKR_OPT_ROW_UNIT_TILES = 1, BKR_OPT_ROW_VEC_POLICY = 2 };
+ *   BKR_OPT_ROW_VEC_POLICY  L2 eviction priority of its z/t neighbour loads: 0 evict_normal, 1 evict_last
+ *   BKR_OPT_ABLATION        bit mask of BKR_ABL_*: parts of the method switched off for the comparison of the paper's
+ *                           Fig. 4 (no block / block BLAS / block BLAS + block Dslash).  Results are
+ *                           the same up to rounding; only the kernels that produce them change.  0 = the full method. */
+enum { BKR_OPT_L2_BUDGET_MB = 0, BKR_OPT_ROW_UNIT_TILES = 1, BKR_OPT_ROW_VEC_POLICY = 2, BKR_OPT_ABLATION = 3 };
+enum {
+    BKR_ABL_UNFUSED_UPDATES = 1, /* Q, P, X updates as separate kernels, X updated right after Alg. 1 l.9 (no deferral)   */
+    BKR_ABL_UNFUSED_GRAM = 2,    /* Q' = Q - MP beta and its Gram matrix as two kernels                                  */
+    BKR_ABL_VECTOR_BLAS = 4,     /* block updates / Gram matrices as N^2 single-vector caxpys / dot products */
+    BKR_ABL_VECTOR_DSLASH = 8    /* the stencil one rhs at a time: links re-read for every rhs         */
+};
 int bkr_set_option(bkr_ctx *ctx, int option, int value);
 
 /* Measured on-chip peaks for the rooflines (not on the hot path).  kind: 0 fp64 FMA, 1 fp32 FMA,

@@ -172,7 +172,8 @@ def cg(dims, fat, lng, mass, b, x0=None, tol=1e-10, maxiter=10000):
 
 def block_cg(dims, fat, lng, mass, B, X0=None, tol=1e-10, maxiter=10000, mixed=False, delta=0.1, ntrace=0):
     """blockCGrQ (Algorithm 1; with mixed=True plus Algorithm 3).  B (N, Vh, 3).
-    returns dict(X, iters, status, reliable_updates, hist, G, C)."""
+    returns dict(X, iters, status, reliable_updates, hist, G, C, QP); G, C, QP = traces of the first ntrace iterations
+    (P^dag M P, C after l.12, and Q^dag P right after l.8: PAPER.md:210)."""
     fat, lng, B = _ca(fat), _ca(lng), _ca(B)
     N = B.shape[0]
     X = np.zeros_like(B) if X0 is None else _ca(X0).copy()
@@ -180,12 +181,13 @@ def block_cg(dims, fat, lng, mass, B, X0=None, tol=1e-10, maxiter=10000, mixed=F
     hist = np.zeros(maxiter + 1)
     tG = np.zeros((max(ntrace, 1), N, N), dtype=np.complex128)
     tC = np.zeros((max(ntrace, 1), N, N), dtype=np.complex128)
+    tQP = np.zeros((max(ntrace, 1), N, N), dtype=np.complex128)
     rc = lib().orc_block_cg(_dims(dims), _ptr(fat), _ptr(lng), ctypes.c_double(mass), N, _ptr(B), _ptr(X),
                             ctypes.c_double(tol), int(maxiter), int(bool(mixed)), ctypes.c_double(delta),
                             ctypes.byref(it), ctypes.byref(nup), hist.ctypes.data_as(_P), int(ntrace), _ptr(tG),
-                            _ptr(tC))
+                            _ptr(tC), _ptr(tQP))
     return dict(X=X, iters=it.value, status=rc, reliable_updates=nup.value, hist=hist[: it.value + 1],
-                G=tG[:ntrace], C=tC[:ntrace])
+                G=tG[:ntrace], C=tC[:ntrace], QP=tQP[:ntrace])
 
 
 def true_relres(dims, fat, lng, mass, B, X):

@@ -358,11 +358,14 @@ static void round_f32(long n, cplx *v)
  * hist (may be NULL): max relative iterated residual, hist[0] initial, hist[it] after it.
  * trace_G / trace_C (may be NULL): G = P^dag M P and C (after l.12) of the first `ntrace`
  * iterations, N*N each, for comparing intermediates (U16).
+ * trace_QP (may be NULL): Q^dag P right after l.8 of the first `ntrace` iterations, Q being the
+ * block that entered l.8 ("Q_old" of PAPER.md:210, whose identity (Q_old)^dag P = 1 pins the
+ * driver, with and without reliable updates).  A trace only: no arithmetic of the solve uses it.
  * Returns 0, -5 on a Cholesky breakdown (U15), -6 at maxiter. */
 int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, int N,
                  const cplx *B, cplx *X, double tol, int maxiter, int mixed, double delta,
                  int *iters, int *nupdates, double *hist, int ntrace, cplx *trace_G,
-                 cplx *trace_C)
+                 cplx *trace_C, cplx *trace_QP)
 {
     if (!dims_ok(D) || N < 1) return -1;
     long V = (long)D[0] * D[1] * D[2] * D[3], Vh = V / 2, L = 3 * Vh, n = L * N;
@@ -410,6 +413,7 @@ int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, 
         orc_block_axpy(L, N, Sd, P, Pn);
         memcpy(P, Pn, sizeof(cplx) * n);
         if (mixed) round_f32(n, P);
+        if (it < ntrace && trace_QP) orc_gram(L, N, Q, P, trace_QP + (long)it * N * N);
         /* l.9  beta = (P^dag M P)^-1 */
         orc_apply_M(D, fin, lin, mass, N, P, AP, T);
         if (mixed) round_f32(n, AP);

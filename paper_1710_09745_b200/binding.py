@@ -16,11 +16,12 @@ LIB_PATH = os.path.join(_HERE, "libbkr.so")
 F64, F32 = 0, 1
 OK, EINVAL, ENOLINKS, ENOMEM, ECUDA, EBREAKDOWN, ENOCONV = 0, -1, -2, -3, -4, -5, -6
 MAX_N = 32
-OPT_L2_BUDGET_MB, OPT_ROW_UNIT_TILES = 0, 1
+OPT_L2_BUDGET_MB, OPT_ROW_UNIT_TILES, OPT_ROW_VEC_POLICY, OPT_ABLATION = 0, 1, 2, 3
+ABL_UNFUSED_UPDATES, ABL_UNFUSED_GRAM, ABL_VECTOR_BLAS, ABL_VECTOR_DSLASH = 1, 2, 4, 8
 
 SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash",
-    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
+    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_update", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
     "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench",
 )
@@ -66,6 +67,7 @@ def lib():
             "bkr_apply_M": (ci, [vp, cd, ci, ci, vp, vp]),
             "bkr_gram": (ci, [vp, ci, ci, vp, vp, ci, vp]),
             "bkr_block_axpy": (ci, [vp, ci, ci, vp, vp, vp]),
+            "bkr_block_update": (ci, [vp, ci, ci, ci, ci, vp, vp, vp, vp]),
             "bkr_block_axpy_gram": (ci, [vp, ci, ci, vp, vp, vp, vp]),
             "bkr_block_qpx_update": (ci, [vp, ci, ci, vp, vp, vp, vp, vp, vp, vp, ci, ci]),
             "bkr_cholesky_upper": (ci, [vp, ci, vp, vp, vp, vp]),
@@ -190,6 +192,14 @@ class Context:
         self._check(lib().bkr_block_axpy(self._h, int(N), int(prec), _dev_ptr(a, "a"), _dev_ptr(X, "X"), _dev_ptr(Y, "Y")),
                     "bkr_block_axpy")
         return Y
+
+    def block_update(self, N, a, C, W, Z, precZ=F64, precW=F64, tri=0):
+        """Z <- C + W a (C may be None); tri 0 general, 1 upper, 2 lower triangular a (bkr.h)."""
+        assert a.dtype == torch.complex128 and tuple(a.shape) == (int(N), int(N))
+        cptr = ctypes.c_void_p(0) if C is None else _dev_ptr(C, "C")
+        self._check(lib().bkr_block_update(self._h, int(N), int(precZ), int(precW), int(tri), _dev_ptr(a, "a"), cptr,
+                                           _dev_ptr(W, "W"), _dev_ptr(Z, "Z")), "bkr_block_update")
+        return Z
 
     def block_axpy_gram(self, N, a, X, Y, prec=F64, out=None):
         """Y += X a and K = Y^dag Y of the updated Y in one pass; returns K (N x N complex128)."""

@@ -56,6 +56,8 @@ int bkr_destroy(bkr_ctx *ctx)
     cudaFree(ctx->tmp_odd[1]);
     cudaFree(ctx->partials);
     cudaFree(ctx->small);
+    cudaFree(ctx->stage[0]);
+    cudaFree(ctx->stage[1]);
     free(ctx);
     return BKR_OK;
 }
@@ -63,9 +65,16 @@ int bkr_destroy(bkr_ctx *ctx)
 int bkr_load_links(bkr_ctx *ctx, const void *fat, const void *lng, int also_f32)
 {
     if (!ctx || !fat || !lng) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     size_t n = link_elems(ctx->g);
     if (!ctx->links64) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->links64, n * sizeof(double2)));
     if (also_f32 && !ctx->links32) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->links32, n * sizeof(float2)));
+    if (!also_f32 && ctx->links32) { // an fp32 copy of the previous links must not survive a reload without one
+        BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->links32);
+        ctx->links32 = nullptr;
+    }
+    solver_invalidate(ctx);
     return launch_pack_links(ctx, (const double2 *)fat, (const double2 *)lng, ctx->links64,
                              also_f32 ? ctx->links32 : nullptr);
 }
@@ -79,18 +88,21 @@ size_t bkr_field_bytes(const bkr_ctx *ctx, int N, int prec)
 int bkr_pack(bkr_ctx *ctx, int N, int prec, const void *canonical, void *native)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !canonical || !native || canonical == native) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     return launch_pack(ctx, N, prec, (const double2 *)canonical, native);
 }
 
 int bkr_unpack(bkr_ctx *ctx, int N, int prec, const void *native, void *canonical)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !canonical || !native || canonical == native) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     return launch_unpack(ctx, N, prec, native, (double2 *)canonical);
 }
 
 int bkr_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !in || !out || in == out) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     if (out_parity != 0 && out_parity != 1) return BKR_EINVAL;
     return launch_dslash(ctx, out_parity, N, prec, in, out, nullptr, 0.0, nullptr);
 }
@@ -98,6 +110,7 @@ int bkr_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, vo
 int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !in || !out || in == out) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     if (!(prec == BKR_F64 ? (void *)ctx->links64 : (void *)ctx->links32)) return BKR_ENOLINKS;
     BKR_TRY(ensure_tmp_odd(ctx, N, prec));
     BKR_TRY(launch_dslash(ctx, 1, N, prec, in, ctx->tmp_odd[prec], nullptr, 0.0, nullptr));
@@ -107,6 +120,7 @@ int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void
 int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, void *K)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !X || !Y || !K) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     int np = 0;
     BKR_TRY(launch_gram_partials(ctx, N, prec, X, Y, hermitian ? 1 : 0, &np, nullptr));
     return launch_gram_finish(ctx, N, np, hermitian ? 1 : 0, (double2 *)K);
@@ -115,12 +129,21 @@ int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int he
 int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !a || !X || !Y || X == Y) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     return launch_block_update(ctx, N, prec, prec, (const double2 *)a, Y, X, Y, nullptr);
+}
+
+int bkr_block_update(bkr_ctx *ctx, int N, int precZ, int precW, int tri, const void *a, const void *C, const void *W, void *Z)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(precZ) || !valid_prec(precW) || tri < 0 || tri > 2 || !a || !W || !Z || W == Z) return BKR_EINVAL;
+    BKR_ENTER(ctx);
+    return launch_block_update(ctx, N, precZ, precW, (const double2 *)a, C, W, Z, nullptr, tri);
 }
 
 int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y, void *K)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !a || !X || !Y || !K || X == Y) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     int np = 0;
     BKR_TRY(launch_update_gram(ctx, N, prec, (const double2 *)a, Y, X, Y, &np, nullptr));
     return launch_gram_finish(ctx, N, np, 1, (double2 *)K);
@@ -130,6 +153,7 @@ int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const 
                          const void *P, void *Pn, void *X, int do_qp, int do_x)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !Sinv || !Sdag || !Wm || !Q || !P || !Pn || !X || P == Pn) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     if (!ctx->api_flags) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->api_flags, sizeof(SolverFlags)));
     SolverFlags f;
     memset(&f, 0, sizeof(f));
@@ -146,6 +170,7 @@ int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const 
 int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, int *status)
 {
     if (!ctx || !valid_n(N) || !H || !R) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     SmallArgs a;
     memset(&a, 0, sizeof(a));
     a.N = N;
@@ -160,6 +185,7 @@ int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, 
 int bkr_hpd_inverse(bkr_ctx *ctx, int N, const void *G, void *Ginv, int *status)
 {
     if (!ctx || !valid_n(N) || !G || !Ginv) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     SmallArgs a;
     memset(&a, 0, sizeof(a));
     a.N = N;
@@ -179,6 +205,7 @@ int bkr_solve_block(bkr_ctx *ctx, double mass, int N, const void *B, void *X, do
                     double delta, double *true_relres, bkr_stats *stats)
 {
     if (!valid_solve(ctx, N, B, X, tol, maxiter) || !valid_prec(inner_prec)) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     if (inner_prec == BKR_F32 && !(delta > 0.0 && delta < 1.0)) return BKR_EINVAL;
     if (!ctx->links64 || (inner_prec == BKR_F32 && !ctx->links32)) return BKR_ENOLINKS;
     int rc = solver_block(ctx, mass, N, (const double2 *)B, (double2 *)X, tol, maxiter, inner_prec, delta, true_relres,
@@ -191,6 +218,7 @@ int bkr_solve_cg(bkr_ctx *ctx, double mass, int N, const void *B, void *X, doubl
                  int *iters, double *true_relres, bkr_stats *stats)
 {
     if (!valid_solve(ctx, N, B, X, tol, maxiter)) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     if (!ctx->links64) return BKR_ENOLINKS;
     int rc = solver_cg(ctx, mass, N, (const double2 *)B, (double2 *)X, tol, maxiter, batched ? 1 : 0, iters,
                        true_relres, stats);
@@ -198,29 +226,37 @@ int bkr_solve_cg(bkr_ctx *ctx, double mass, int N, const void *B, void *X, doubl
     return rc;
 }
 
-// host-buffer variants: staging through two device blocks owned by the call
+// host-buffer variants: staging through two device blocks the context keeps between calls (no allocation in the timed
+// end-to-end region after the first call for a given N)
 static int with_host_buffers(bkr_ctx *ctx, int N, const void *B_host, void *X_host, double2 **dB, double2 **dX)
 {
-    size_t bytes = field_elems(ctx->g, N) * sizeof(double2);
-    *dB = *dX = nullptr;
-    BKR_CUDA(ctx, cudaMalloc((void **)dB, bytes));
-    if (cudaMalloc((void **)dX, bytes) != cudaSuccess) {
-        cudaFree(*dB);
-        *dB = nullptr;
-        return BKR_ENOMEM;
+    const size_t bytes = field_elems(ctx->g, N) * sizeof(double2);
+    if (ctx->stage_bytes < bytes) {
+        cudaFree(ctx->stage[0]);
+        cudaFree(ctx->stage[1]);
+        ctx->stage[0] = ctx->stage[1] = nullptr;
+        ctx->stage_bytes = 0;
+        BKR_CUDA(ctx, cudaMalloc((void **)&ctx->stage[0], bytes));
+        if (cudaMalloc((void **)&ctx->stage[1], bytes) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(ctx->stage[0]);
+            ctx->stage[0] = nullptr;
+            return BKR_ENOMEM;
+        }
+        ctx->stage_bytes = bytes;
     }
+    *dB = ctx->stage[0];
+    *dX = ctx->stage[1];
     BKR_CUDA(ctx, cudaMemcpyAsync(*dB, B_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
     BKR_CUDA(ctx, cudaMemcpyAsync(*dX, X_host, bytes, cudaMemcpyHostToDevice, ctx->stream));
     return BKR_OK;
 }
 
-static int finish_host_buffers(bkr_ctx *ctx, int N, void *X_host, double2 *dB, double2 *dX, int rc)
+static int finish_host_buffers(bkr_ctx *ctx, int N, void *X_host, double2 *dX, int rc)
 {
-    size_t bytes = field_elems(ctx->g, N) * sizeof(double2);
+    const size_t bytes = field_elems(ctx->g, N) * sizeof(double2);
     cudaError_t e = cudaMemcpyAsync(X_host, dX, bytes, cudaMemcpyDeviceToHost, ctx->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-    cudaFree(dB);
-    cudaFree(dX);
     if (e != cudaSuccess) {
         ctx->last_cuda = (int)e;
         return BKR_ECUDA;
@@ -232,25 +268,28 @@ int bkr_solve_block_host(bkr_ctx *ctx, double mass, int N, const void *B_host, v
                          int inner_prec, double delta, double *true_relres, bkr_stats *stats)
 {
     if (!valid_solve(ctx, N, B_host, X_host, tol, maxiter)) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     double2 *dB, *dX;
     BKR_TRY(with_host_buffers(ctx, N, B_host, X_host, &dB, &dX));
     int rc = bkr_solve_block(ctx, mass, N, dB, dX, tol, maxiter, inner_prec, delta, true_relres, stats);
-    return finish_host_buffers(ctx, N, X_host, dB, dX, rc);
+    return finish_host_buffers(ctx, N, X_host, dX, rc);
 }
 
 int bkr_solve_cg_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void *X_host, double tol, int maxiter,
                       int batched, int *iters, double *true_relres, bkr_stats *stats)
 {
     if (!valid_solve(ctx, N, B_host, X_host, tol, maxiter)) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     double2 *dB, *dX;
     BKR_TRY(with_host_buffers(ctx, N, B_host, X_host, &dB, &dX));
     int rc = bkr_solve_cg(ctx, mass, N, dB, dX, tol, maxiter, batched, iters, true_relres, stats);
-    return finish_host_buffers(ctx, N, X_host, dB, dX, rc);
+    return finish_host_buffers(ctx, N, X_host, dX, rc);
 }
 
 int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void *B, int iters, long long *launches)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !B || iters < 0) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     if (!ctx->links64 || (prec == BKR_F32 && !ctx->links32)) return BKR_ENOLINKS;
     return solver_bench_iterations(ctx, mass, N, prec, (const double2 *)B, iters, launches);
 }
@@ -258,6 +297,7 @@ int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void 
 int bkr_microbench(bkr_ctx *ctx, int kind, int reps, double *result)
 {
     if (!ctx) return BKR_EINVAL;
+    BKR_ENTER(ctx);
     return run_microbench(ctx, kind, reps, result);
 }
 
@@ -286,6 +326,7 @@ int bkr_set_option(bkr_ctx *ctx, int option, int value)
     case BKR_OPT_L2_BUDGET_MB: ctx->l2_budget_mb = value; break;
     case BKR_OPT_ROW_UNIT_TILES: ctx->row_unit_tiles = value; break;
     case BKR_OPT_ROW_VEC_POLICY: ctx->row_vec_policy = value; break;
+    case BKR_OPT_ABLATION: ctx->ablation = value & 15; break;
     default: return BKR_EINVAL;
     }
     // blocking tables are rebuilt on the next stencil call

@@ -65,6 +65,7 @@ struct bkr_ctx {
     int row_nstrip, row_key;
     int dslash_force; // bkr_set_dslash_variant: -1 automatic, 0 plain, 1 window, 2 row window
     int l2_budget_mb, row_unit_tiles, row_vec_policy; // bkr_set_option (0 = built-in default)
+    int ablation;       // BKR_OPT_ABLATION bit mask (bkr.h): 0 = the full method
     SolverFlags *api_flags; // device flags for the API-level fused update
     int dslash_nblock;  // rhs count of the whole block while launch_dslash works through it in chunks (L2 blocking uses it)
     int dslash_variant; // last stencil kernel used: 0 plain, 1 window, -1 none yet
@@ -78,6 +79,9 @@ struct bkr_ctx {
     double2 *small;
     // solver workspace (allocated on first solve for a given N / precision, reused)
     struct Workspace *ws;
+    // device staging blocks of the host-buffer entry points (kept between calls)
+    double2 *stage[2];
+    size_t stage_bytes;
 };
 
 #define BKR_CUDA(ctx, call)                                   \
@@ -87,6 +91,12 @@ struct bkr_ctx {
             (ctx)->last_cuda = (int)e_;                       \
             return e_ == cudaErrorMemoryAllocation ? BKR_ENOMEM : BKR_ECUDA; \
         }                                                     \
+    } while (0)
+
+// every ABI entry makes the context's device current (a context may live on any device of the process)
+#define BKR_ENTER(ctx)                                                          \
+    do {                                                                        \
+        if (cudaSetDevice((ctx)->device) != cudaSuccess) return BKR_ECUDA;      \
     } while (0)
 
 #define BKR_TRY(call)                 \
@@ -140,14 +150,11 @@ int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, dou
 // tri: 0 = general a, 1 = a upper triangular, 2 = a lower triangular (entries on the other side are not read).
 int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C,
                         const void *W, void *Z, const int *done, int tri = 0);
-// Deferred X update fused with the P update (Alg. 1 l.10 of the previous iteration + l.8 of this one):
-//   if (flags->xpend)  X  += P Wm          (X fp64, in place)
-//   if (!flags->done)  Pn  = Q + P Sdag    (Pn must not alias P)
-// one pass over P for both products.  prec = precision of P, Q, Pn.
-int launch_px_update(bkr_ctx *ctx, int N, int prec, const double2 *Sdag, const double2 *Wm, const void *Q, const void *P,
-                     void *Pn, double2 *X, const SolverFlags *flags);
-// The same with Alg. 2 l.4 of the previous iteration folded in (if !flags->done):  Q = Q Sinv (in place; Sinv upper
-// triangular, S^dag lower triangular: zero fragments skipped), Pn = Q + P Sdag;  X += P Wm if flags->xpend.
+// Fused update at the top of an iteration (the X update of Alg. 1 l.10 deferred into the next iteration's
+// l.8; Alg. 2 l.4 of the previous iteration folded in as well), one pass over Q, P, X:
+//   if (!flags->done)  Q = Q Sinv (in place; Sinv upper triangular),  Pn = Q + P Sdag (S^dag lower triangular; zero
+//                      fragments skipped; Pn must not alias P)
+//   if (flags->xpend)  X += P Wm   (X fp64, in place).      prec = precision of P, Q, Pn.
 int launch_pqx_update(bkr_ctx *ctx, int N, int prec, const double2 *Sinv, const double2 *Sdag, const double2 *Wm, void *Q,
                       const void *P, void *Pn, double2 *X, const SolverFlags *flags);
 // Alg. 1 l.11 + Alg. 2 l.2 fused: Z = C + W a and stage 1 of H = Z^dag Z (Hermitian) in one pass; all blocks precision prec.
@@ -203,5 +210,6 @@ int solver_cg(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, do
 int solver_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const double2 *B, int iters,
                             long long *launches);
 void solver_free_workspace(bkr_ctx *ctx);
+void solver_invalidate(bkr_ctx *ctx); // links changed: cached bench state is stale
 int ensure_partials(bkr_ctx *ctx, size_t bytes);
 int ensure_tmp_odd(bkr_ctx *ctx, int N, int prec);

@@ -273,13 +273,13 @@ static int launch_tg(bkr_ctx *ctx, int parity, int N, const void *in, void *out,
     const int opts = oenv ? atoi(oenv) : 0;
     dim3 block(BKR_LINK_TILE, G);
     unsigned grid = (unsigned)std::min(ntiles, BKR_NUM_SMS * MINB);
-    static bool attr_done = false; // one flag per instantiation
-    if (!attr_done) {
+    static int attr_dev = -1; // per instantiation: the opt-in is per device
+    if (attr_dev != ctx->device) {
         BKR_CUDA(ctx, cudaFuncSetAttribute(dslash_kernel<Real, T, G, true, MINB, DD, RG>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
         BKR_CUDA(ctx, cudaFuncSetAttribute(dslash_kernel<Real, T, G, false, MINB, DD, RG>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-        attr_done = true;
+        attr_dev = ctx->device;
     }
     if (N == T * G)
         dslash_kernel<Real, T, G, true, MINB, DD, RG><<<grid, block, SMEM, ctx->stream>>>(

@@ -547,7 +547,7 @@ static int launch_row_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     p.dry = ctx->row_vec_policy == 64;
 
     auto kern = dslash_row_kernel<Real, T, C, XP, XH>;
-    static int max_clusters = -1; // per instantiation
+    static int max_clusters = -1, attr_dev = -1; // per instantiation; the shared-memory opt-in is per device
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cudaLaunchAttribute attr[1];
@@ -560,7 +560,8 @@ static int launch_row_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     cfg.stream = ctx->stream;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (max_clusters < 0) {
+    if (max_clusters < 0 || attr_dev != ctx->device) {
+        attr_dev = ctx->device;
         BKR_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ROW_SMEM_MAX));
         cfg.gridDim = dim3((BKR_NUM_SMS / C) * C);
         int n = 0;

@@ -251,13 +251,13 @@ static int update_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const void
     if (rp.nstg < 2) return BKR_EINVAL;
     const size_t ntiles = (L + rp.R - 1) / rp.R;
     const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
-    static bool attr_done = false; // one flag per instantiation
-    if (!attr_done) {
+    static int attr_dev = -1; // per instantiation: the opt-in is per device
+    if (attr_dev != ctx->device) {
         BKR_CUDA(ctx, cudaFuncSetAttribute(update_tma_kernel<RealZ, RealW, NTJ, NIS, true, CW>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));
         BKR_CUDA(ctx, cudaFuncSetAttribute(update_tma_kernel<RealZ, RealW, NTJ, NIS, false, CW>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));
-        attr_done = true;
+        attr_dev = ctx->device;
     }
     if (C)
         update_tma_kernel<RealZ, RealW, NTJ, NIS, true, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
@@ -469,11 +469,11 @@ static int gram_go(bkr_ctx *ctx, size_t L, int N, const void *X, const void *Y, 
     const unsigned gx = (unsigned)(ntiles < (size_t)GRAM_MAX_GRID ? ntiles : (size_t)GRAM_MAX_GRID);
 #define GRAM_LAUNCH(H_, A_, TIB_, GRID_)                                                                               \
     do {                                                                                                               \
-        static bool attr_done = false;                                                                                 \
-        if (!attr_done) {                                                                                              \
+        static int attr_dev = -1; /* per instantiation: the opt-in is per device */                                   \
+        if (attr_dev != ctx->device) {                                                                                              \
             BKR_CUDA(ctx, cudaFuncSetAttribute(gram_tma_kernel<Real, NT, H_, A_, TIB_, CW>,                            \
                                                cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));          \
-            attr_done = true;                                                                                          \
+            attr_dev = ctx->device;                                                                                          \
         }                                                                                                              \
         gram_tma_kernel<Real, NT, H_, A_, TIB_, CW><<<GRID_, (CW + 1) * 32, rp.smem, ctx->stream>>>(L, N, rp, x, y,     \
                                                                                                    ctx->partials, done); \
@@ -510,157 +510,19 @@ int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const voi
 #undef GRAM_NT
 }
 
-// ------------------------------------------------------------------------------------------ fused P / X update
-// Alg. 1 l.8 of this iteration and l.10 of the previous one in one pass over P (the deferral of PAPER.md:243):
+// ------------------------------------------------------------------------------------------ fused Q / P / X update
+// Alg. 2 l.4 of the previous iteration, Alg. 1 l.8 of this one and l.10 of the previous one in one pass over Q', P, X
+// (the deferral of PAPER.md:243):
+//     Q   = Q' Si     if !flags->done   (Si = S^-1 upper triangular; in place)
+//     Pn  = Q + P Sd  if !flags->done   (Sd = S^dag lower triangular)
 //     X  += P Wm      if flags->xpend   (Wm = beta C of the previous l.9; X fp64, in place)
-//     Pn  = Q + P Sd  if !flags->done   (Sd = S^dag)
-// Reads P, Q, X and writes Pn, X: 5 block passes instead of the 6 of two update_tma_kernel launches.  Same ring,
-// fragment layouts and DMMA tiles as update_tma_kernel; a stage holds R rows of P (A-fragment layout), of Q and of X
-// (accumulator layout).
+// 6 block passes.  Same ring, fragment layouts and DMMA tiles as update_tma_kernel; a stage holds R rows of Q' and P
+// (A-fragment layout) and of X (accumulator layout).
 struct Ring3 {
     int R, nstg;
     uint32_t rs_p, rs_q, rs_x, off_q, off_x, stage_bytes, off_ring;
     size_t smem;
 };
-
-template <typename RealP, int NTJ, int NIS, int CW>
-__global__ void __launch_bounds__((CW + 1) * 32, 1)
-px_update_kernel(size_t L, int N, Ring3 rp, const double2 *__restrict__ Sd, const double2 *__restrict__ Wm,
-                 const typename CxT<RealP>::type *__restrict__ Q, const typename CxT<RealP>::type *__restrict__ P,
-                 typename CxT<RealP>::type *__restrict__ Pn, double2 *X, const SolverFlags *fl)
-{
-    typedef typename CxT<RealP>::type CxP;
-    constexpr int NF = NIS * NTJ * 32;
-    extern __shared__ __align__(128) unsigned char dsm[];
-    uint64_t *full = reinterpret_cast<uint64_t *>(dsm);
-    uint64_t *empty = full + MB_MAX_STAGES;
-    double *b1r = reinterpret_cast<double *>(dsm + 128), *b1i = b1r + NF, *b2r = b1i + NF, *b2i = b2r + NF;
-    unsigned char *ring = dsm + rp.off_ring;
-    const bool doX = fl->xpend != 0, doP = fl->done == 0;
-    if (!doX && !doP) return;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < rp.nstg; s++) {
-            mbar_init(&full[s], 1);
-            mbar_init(&empty[s], CW);
-        }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    for (int idx = threadIdx.x; idx < NF; idx += blockDim.x) {
-        const int ln = idx & 31, f = idx >> 5;
-        const int is = f / NTJ, tj = f % NTJ;
-        const int i = 4 * is + (ln & 3), j = 8 * tj + (ln >> 2);
-        const bool in = i < N && j < N;
-        const double2 v1 = in ? Sd[i * N + j] : make_double2(0.0, 0.0), v2 = in ? Wm[i * N + j] : make_double2(0.0, 0.0);
-        b1r[idx] = v1.x;
-        b1i[idx] = v1.y;
-        b2r[idx] = v2.x;
-        b2i[idx] = v2.y;
-    }
-    __syncthreads();
-
-    const size_t ntiles = (L + rp.R - 1) / rp.R;
-    const int my = (int)((ntiles > blockIdx.x) ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0);
-
-    if (warp == CW) { // ---------------- producer
-        const uint64_t pol = policy_evict_first();
-        for (int it = 0; it < my; it++) {
-            const int s = it % rp.nstg;
-            if (it >= rp.nstg) mbar_wait(&empty[s], ((it / rp.nstg) - 1) & 1);
-            const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
-            const uint32_t rows = (uint32_t)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
-            unsigned char *st = ring + (size_t)s * rp.stage_bytes;
-            if (lane == 0)
-                mbar_expect_tx(&full[s], (uint32_t)N * rows *
-                                             (uint32_t)(sizeof(CxP) + (doP ? sizeof(CxP) : 0) + (doX ? sizeof(double2) : 0)));
-            __syncwarp();
-            if (lane < N) {
-                tma_load_1d_hint(st + (size_t)lane * rp.rs_p, P + (size_t)lane * L + r0, rows * (uint32_t)sizeof(CxP), &full[s], pol);
-                if (doP)
-                    tma_load_1d_hint(st + rp.off_q + (size_t)lane * rp.rs_q, Q + (size_t)lane * L + r0,
-                                     rows * (uint32_t)sizeof(CxP), &full[s], pol);
-                if (doX)
-                    tma_load_1d_hint(st + rp.off_x + (size_t)lane * rp.rs_x, X + (size_t)lane * L + r0,
-                                     rows * (uint32_t)sizeof(double2), &full[s], pol);
-            }
-        }
-        return;
-    }
-
-    // ---------------- consumers
-    const int m = lane >> 2, q = lane & 3;
-    for (int it = 0; it < my; it++) {
-        const int s = it % rp.nstg;
-        const size_t r0 = ((size_t)blockIdx.x + (size_t)it * gridDim.x) * rp.R;
-        const int rows = (int)((L - r0 < (size_t)rp.R) ? L - r0 : rp.R);
-        const unsigned char *stP = ring + (size_t)s * rp.stage_bytes;
-        const unsigned char *stQ = stP + rp.off_q, *stX = stP + rp.off_x;
-        mbar_wait_acq(&full[s], (it / rp.nstg) & 1);
-        for (int u = warp; u < rows / 8; u += CW) {
-            const int row = 8 * u + m;
-            double2 wf[NIS];
-#pragma unroll
-            for (int is = 0; is < NIS; is++) {
-                const int i = 4 * is + q;
-                wf[is] = i < N ? sm_cx<CxP>(stP + (size_t)i * rp.rs_p + (size_t)row * sizeof(CxP)) : make_double2(0.0, 0.0);
-            }
-            if (doP) {
-                double zre[NTJ][2], zim[NTJ][2];
-#pragma unroll
-                for (int tj = 0; tj < NTJ; tj++) zre[tj][0] = zre[tj][1] = zim[tj][0] = zim[tj][1] = 0.0;
-#pragma unroll
-                for (int is = 0; is < NIS; is++)
-#pragma unroll
-                    for (int tj = 0; tj < NTJ; tj++) {
-                        const int f = (is * NTJ + tj) * 32 + lane;
-                        const double br = b1r[f], bi = b1i[f];
-                        dmma(zre[tj], wf[is].x, br);
-                        dmma(zre[tj], wf[is].y, -bi);
-                        dmma(zim[tj], wf[is].x, bi);
-                        dmma(zim[tj], wf[is].y, br);
-                    }
-#pragma unroll
-                for (int tj = 0; tj < NTJ; tj++)
-#pragma unroll
-                    for (int r = 0; r < 2; r++) {
-                        const int j = 8 * tj + 2 * q + r;
-                        if (j < N) {
-                            const double2 c = sm_cx<CxP>(stQ + (size_t)j * rp.rs_q + (size_t)row * sizeof(CxP));
-                            st_cx<CxP>(Pn + (size_t)j * L + r0 + row, zre[tj][r] + c.x, zim[tj][r] + c.y);
-                        }
-                    }
-            }
-            if (doX) {
-                double zre[NTJ][2], zim[NTJ][2];
-#pragma unroll
-                for (int tj = 0; tj < NTJ; tj++) zre[tj][0] = zre[tj][1] = zim[tj][0] = zim[tj][1] = 0.0;
-#pragma unroll
-                for (int is = 0; is < NIS; is++)
-#pragma unroll
-                    for (int tj = 0; tj < NTJ; tj++) {
-                        const int f = (is * NTJ + tj) * 32 + lane;
-                        const double br = b2r[f], bi = b2i[f];
-                        dmma(zre[tj], wf[is].x, br);
-                        dmma(zre[tj], wf[is].y, -bi);
-                        dmma(zim[tj], wf[is].x, bi);
-                        dmma(zim[tj], wf[is].y, br);
-                    }
-#pragma unroll
-                for (int tj = 0; tj < NTJ; tj++)
-#pragma unroll
-                    for (int r = 0; r < 2; r++) {
-                        const int j = 8 * tj + 2 * q + r;
-                        if (j < N) {
-                            const double2 c = sm_cx<double2>(stX + (size_t)j * rp.rs_x + (size_t)row * sizeof(double2));
-                            st_cx<double2>(X + (size_t)j * L + r0 + row, zre[tj][r] + c.x, zim[tj][r] + c.y);
-                        }
-                    }
-            }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive_rel(&empty[s]);
-    }
-}
 
 template <typename RealP, int NTJ, int NIS, int CW>
 __global__ void __launch_bounds__((CW + 1) * 32, 1)
@@ -834,69 +696,6 @@ pqx_update_kernel(size_t L, int N, Ring3 rp, const double2 *__restrict__ Si, con
 }
 
 template <typename RealP, int NTJ, int NIS>
-static int px_go(bkr_ctx *ctx, size_t L, int N, const double2 *Sd, const double2 *Wm, const void *Q, const void *P, void *Pn,
-                 double2 *X, const SolverFlags *fl)
-{
-    typedef typename CxT<RealP>::type CxP;
-    constexpr int CW = 8;
-    const size_t fixed = (128 + (size_t)4 * NIS * NTJ * 32 * sizeof(double) + 127) / 128 * 128;
-    Ring3 rp;
-    memset(&rp, 0, sizeof(rp));
-    for (int R = 512; R >= 32; R /= 2) {
-        rp.R = R;
-        rp.rs_p = (uint32_t)(R * sizeof(CxP) + 32);
-        rp.rs_q = (uint32_t)(R * sizeof(CxP) + 16);
-        rp.rs_x = (uint32_t)(R * sizeof(double2) + 16);
-        rp.off_q = ((uint32_t)N * rp.rs_p + 127) / 128 * 128;
-        rp.off_x = (rp.off_q + (uint32_t)N * rp.rs_q + 127) / 128 * 128;
-        rp.stage_bytes = (rp.off_x + (uint32_t)N * rp.rs_x + 127) / 128 * 128;
-        rp.off_ring = (uint32_t)fixed;
-        int n = (int)((MB_SMEM_BUDGET - fixed) / rp.stage_bytes);
-        if (n > MB_MAX_STAGES) n = MB_MAX_STAGES;
-        rp.nstg = n;
-        rp.smem = fixed + (size_t)n * rp.stage_bytes;
-        if ((n >= 4 && (L + R - 1) / R >= (size_t)2 * BKR_NUM_SMS) || R == 32) break;
-    }
-    if (rp.nstg < 2) return BKR_EINVAL;
-    const size_t ntiles = (L + rp.R - 1) / rp.R;
-    const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
-    static bool attr_done = false; // one flag per instantiation
-    if (!attr_done) {
-        BKR_CUDA(ctx, cudaFuncSetAttribute(px_update_kernel<RealP, NTJ, NIS, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           MB_SMEM_BUDGET));
-        attr_done = true;
-    }
-    px_update_kernel<RealP, NTJ, NIS, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
-        L, N, rp, Sd, Wm, (const CxP *)Q, (const CxP *)P, (CxP *)Pn, X, fl);
-    return bkr_check_launch(ctx);
-}
-
-template <typename RealP>
-static int launch_px_t(bkr_ctx *ctx, int N, const double2 *Sd, const double2 *Wm, const void *Q, const void *P, void *Pn,
-                       double2 *X, const SolverFlags *fl)
-{
-    const size_t L = (size_t)ctx->g.Vh * 3;
-#define PX_GO(NTJ_, NIS_) return px_go<RealP, NTJ_, NIS_>(ctx, L, N, Sd, Wm, Q, P, Pn, X, fl)
-    switch ((N + 3) / 4) {
-    case 1: PX_GO(1, 1);
-    case 2: PX_GO(1, 2);
-    case 3: PX_GO(2, 3);
-    case 4: PX_GO(2, 4);
-    case 5: PX_GO(3, 5);
-    case 6: PX_GO(3, 6);
-    case 7: PX_GO(4, 7);
-    default: PX_GO(4, 8);
-    }
-#undef PX_GO
-}
-
-int launch_px_update(bkr_ctx *ctx, int N, int prec, const double2 *Sdag, const double2 *Wm, const void *Q, const void *P,
-                     void *Pn, double2 *X, const SolverFlags *flags)
-{
-    if (prec == BKR_F64) return launch_px_t<double>(ctx, N, Sdag, Wm, Q, P, Pn, X, flags);
-    return launch_px_t<float>(ctx, N, Sdag, Wm, Q, P, Pn, X, flags);
-}
-template <typename RealP, int NTJ, int NIS>
 static int pqx_go(bkr_ctx *ctx, size_t L, int N, const double2 *Si, const double2 *Sd, const double2 *Wm, void *Q, const void *P, void *Pn,
                  double2 *X, const SolverFlags *fl)
 {
@@ -923,11 +722,11 @@ static int pqx_go(bkr_ctx *ctx, size_t L, int N, const double2 *Si, const double
     if (rp.nstg < 2) return BKR_EINVAL;
     const size_t ntiles = (L + rp.R - 1) / rp.R;
     const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
-    static bool attr_done = false; // one flag per instantiation
-    if (!attr_done) {
+    static int attr_dev = -1; // per instantiation: the opt-in is per device
+    if (attr_dev != ctx->device) {
         BKR_CUDA(ctx, cudaFuncSetAttribute(pqx_update_kernel<RealP, NTJ, NIS, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            MB_SMEM_BUDGET));
-        attr_done = true;
+        attr_dev = ctx->device;
     }
     pqx_update_kernel<RealP, NTJ, NIS, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
         L, N, rp, Si, Sd, Wm, (CxP *)Q, (const CxP *)P, (CxP *)Pn, X, fl);
@@ -1138,11 +937,11 @@ static int update_gram_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const
     const size_t ntiles = (L + rp.R - 1) / rp.R;
     const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
     BKR_TRY(ensure_partials(ctx, (size_t)2 * BKR_NUM_SMS * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
-    static bool attr_done = false; // one flag per instantiation
-    if (!attr_done) {
+    static int attr_dev = -1; // per instantiation: the opt-in is per device
+    if (attr_dev != ctx->device) {
         BKR_CUDA(ctx, cudaFuncSetAttribute(update_gram_kernel<Real, NT, NIS, CW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            MB_SMEM_BUDGET));
-        attr_done = true;
+        attr_dev = ctx->device;
     }
     update_gram_kernel<Real, NT, NIS, CW><<<grid, (CW + 1) * 32, rp.smem, ctx->stream>>>(
         L, N, rp, (uint32_t)off_red, a, (const Cx *)C, (const Cx *)W, (Cx *)Z, ctx->partials, done);

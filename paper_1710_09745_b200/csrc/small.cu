@@ -315,11 +315,11 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
 int launch_small(bkr_ctx *ctx, const SmallArgs &args)
 {
     size_t smem = (size_t)4 * args.N * args.N * sizeof(double2);
-    static bool attr_set = false;
-    if (!attr_set) {
+    static int attr_dev = -1; // the opt-in is per device
+    if (attr_dev != ctx->device) {
         cudaFuncSetAttribute(small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
-        attr_set = true;
+        attr_dev = ctx->device;
     }
     small_kernel<<<1, 256, smem, ctx->stream>>>(args);
     return bkr_check_launch(ctx);

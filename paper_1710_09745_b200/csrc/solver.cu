@@ -22,7 +22,7 @@ struct Workspace {
     double2 *cg_r, *cg_p, *cg_q;
     int cgN;
     cudaEvent_t ev0, ev1;
-    bool bench_ready;
+    bool bench_ready, have_block, have_cg;
 };
 
 static void free_ws(Workspace *w)
@@ -57,8 +57,23 @@ int ensure_tmp_odd(bkr_ctx *ctx, int N, int prec)
     return BKR_OK;
 }
 
-// common small allocations; blocks are allocated by the block / CG entry points as they need them
+static int get_ws_alloc(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fields);
+
+// common small allocations; blocks are allocated by the block / CG entry points as they need them.  A failed allocation
+// frees the whole workspace: the next call starts from scratch instead of running kernels on half of the blocks.
 static int get_ws(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fields)
+{
+    const int rc = get_ws_alloc(ctx, N, prec, block_fields, cg_fields);
+    if (rc != BKR_OK) solver_free_workspace(ctx);
+    return rc;
+}
+
+void solver_invalidate(bkr_ctx *ctx)
+{
+    if (ctx->ws) ctx->ws->bench_ready = false;
+}
+
+static int get_ws_alloc(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fields)
 {
     Workspace *w = ctx->ws;
     if (w && (w->N != N || w->prec != prec)) {
@@ -91,7 +106,7 @@ static int get_ws(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fiel
         BKR_CUDA(ctx, cudaMalloc((void **)&w->Bn, w->bytes64));
         BKR_CUDA(ctx, cudaMalloc((void **)&w->Xn, w->bytes64));
     }
-    if (block_fields && !w->Q) {
+    if (block_fields && !w->have_block) {
         BKR_CUDA(ctx, cudaMalloc(&w->Q, w->bytesP));
         BKR_CUDA(ctx, cudaMalloc(&w->Q2, w->bytesP));
         BKR_CUDA(ctx, cudaMalloc(&w->P, w->bytesP));
@@ -101,11 +116,13 @@ static int get_ws(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fiel
             BKR_CUDA(ctx, cudaMalloc((void **)&w->Y, w->bytes64));
             BKR_CUDA(ctx, cudaMalloc((void **)&w->R64, w->bytes64));
         } else w->R64 = (double2 *)w->AP;
+        w->have_block = true;
     }
-    if (cg_fields && !w->cg_r) {
+    if (cg_fields && !w->have_cg) {
         BKR_CUDA(ctx, cudaMalloc((void **)&w->cg_r, w->bytes64));
         BKR_CUDA(ctx, cudaMalloc((void **)&w->cg_p, w->bytes64));
         BKR_CUDA(ctx, cudaMalloc((void **)&w->cg_q, w->bytes64));
+        w->have_cg = true;
     }
     BKR_TRY(ensure_tmp_odd(ctx, N, BKR_F64));
     if (prec != BKR_F64) BKR_TRY(ensure_tmp_odd(ctx, N, prec));
@@ -114,8 +131,57 @@ static int get_ws(bkr_ctx *ctx, int N, int prec, bool block_fields, bool cg_fiel
 
 static int apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out, const int *done)
 {
+    if (ctx->ablation & BKR_ABL_VECTOR_DSLASH) {
+        // Fig. 4 "no block Dslash" arm: one single-rhs stencil call per vector, links re-read N times
+        const size_t stride = (size_t)3 * ctx->g.Vh * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
+        for (int j = 0; j < N; j++) {
+            const char *vi = (const char *)in + j * stride;
+            char *vt = (char *)ctx->tmp_odd[prec] + j * stride, *vo = (char *)out + j * stride;
+            BKR_TRY(launch_dslash(ctx, 1, 1, prec, vi, vt, nullptr, 0.0, done));
+            BKR_TRY(launch_dslash(ctx, 0, 1, prec, vt, vo, vi, 4.0 * mass * mass, done));
+        }
+        return BKR_OK;
+    }
     BKR_TRY(launch_dslash(ctx, 1, N, prec, in, ctx->tmp_odd[prec], nullptr, 0.0, done));
     return launch_dslash(ctx, 0, N, prec, ctx->tmp_odd[prec], out, in, 4.0 * mass * mass, done);
+}
+
+// Block update / Gram as the solver calls them.  With BKR_ABL_VECTOR_BLAS they run as N^2 single-vector caxpys and dot
+// products -- the "no block BLAS" arm of the paper's Fig. 4 (quadratic memory traffic); the
+// structural zeros of triangular coefficients are still skipped.
+static int blk_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C, const void *W, void *Z,
+                      const int *done, int tri)
+{
+    if (!(ctx->ablation & BKR_ABL_VECTOR_BLAS)) return launch_block_update(ctx, N, precZ, precW, a, C, W, Z, done, tri);
+    const size_t L = (size_t)3 * ctx->g.Vh;
+    const size_t sz = L * (precZ == BKR_F64 ? sizeof(double2) : sizeof(float2)), sw = L * (precW == BKR_F64 ? sizeof(double2) : sizeof(float2));
+    for (int j = 0; j < N; j++) {
+        char *zj = (char *)Z + j * sz;
+        const char *cj = C ? (const char *)C + j * sz : nullptr;
+        bool first = true;
+        for (int i = 0; i < N; i++) {
+            if ((tri == 1 && i > j) || (tri == 2 && i < j)) continue;
+            BKR_TRY(launch_block_update(ctx, 1, precZ, precW, a + (size_t)i * N + j, first ? (const void *)cj : (const void *)zj,
+                                        (const char *)W + i * sw, zj, done, 0));
+            first = false;
+        }
+    }
+    return BKR_OK;
+}
+
+// stage 1 of a Hermitian Gram matrix K = X^dag Y; *np = number of partials, 0 when K itself is already in ctx->small
+static int blk_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int *np, const int *done)
+{
+    if (!(ctx->ablation & BKR_ABL_VECTOR_BLAS)) return launch_gram_partials(ctx, N, prec, X, Y, 1, np, done);
+    const size_t sv = (size_t)3 * ctx->g.Vh * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
+    for (int i = 0; i < N; i++)
+        for (int j = i; j < N; j++) {
+            int n1 = 0;
+            BKR_TRY(launch_gram_partials(ctx, 1, prec, (const char *)X + i * sv, (const char *)Y + j * sv, 0, &n1, done));
+            BKR_TRY(launch_gram_finish(ctx, 1, n1, 0, ctx->small + (size_t)i * N + j));
+        }
+    *np = 0;
+    return BKR_OK;
 }
 
 static int read_flags(bkr_ctx *ctx, Workspace *w)
@@ -135,6 +201,7 @@ static SmallArgs small_args(Workspace *w, int mode, int num_partials, double tol
     a.mode = mode;
     a.num_partials = num_partials;
     a.partials = ctx->partials;
+    a.in = ctx->small; // used when num_partials == 0 (BKR_ABL_VECTOR_BLAS: the Gram matrix was assembled entry by entry)
     a.C = w->C; a.Cprev = w->Cprev; a.negbeta = w->negbeta; a.W = w->W; a.Sinv = w->Sinv; a.Sdag = w->Sdag;
     a.bnorm2 = w->bnorm2;
     a.tol = tol; a.delta = delta;
@@ -148,15 +215,15 @@ __global__ void set_identity_kernel(int N, double2 *A)
     for (int o = threadIdx.x; o < N * N; o += blockDim.x) A[o] = make_double2(o / N == o % N ? 1.0 : 0.0, 0.0);
 }
 
-// BKR_NO_QFUSE=1 (comparison runs): Q = Q' S^-1 as its own kernel at the end of the iteration
-// Fused updates only up to 24 rhs: beyond, the update kernels are bound by the FP64 tensor pipe, the fused ones spill,
-// and separate kernels are faster (32^4, N = 32: 5.39 vs 5.58 ms per iteration; N = 24: 3.82 vs 3.76 ms).
+// Fused Q / P / X update (pqx_update_kernel) only up to 24 rhs: beyond, the update kernels are bound by the FP64 tensor
+// pipe, the fused ones spill, and separate kernels are faster (32^4, N = 32: 5.39 vs 5.58 ms per iteration; N = 24: 3.82
+// vs 3.76 ms).  BKR_ABL_UNFUSED_UPDATES (Fig. 4-style comparison runs) switches it off: five separate passes, X updated
+// right after l.9 as in the unfused Algorithm 1.
 static const int FUSE_MAX_N = 24;
 
-static bool fuse_q(int N)
+static bool fuse_qpx(const bkr_ctx *ctx, int N)
 {
-    static const bool f = getenv("BKR_NO_QFUSE") == nullptr && getenv("BKR_NO_DEFER") == nullptr;
-    return f && N <= FUSE_MAX_N;
+    return N <= FUSE_MAX_N && !(ctx->ablation & (BKR_ABL_UNFUSED_UPDATES | BKR_ABL_VECTOR_BLAS));
 }
 
 // Alg. 1 l.3-l.6 (and Alg. 3 l.4-l.6 when relupd): R = B - M Xcur in fp64, thin QR, Q in inner precision, P kept.
@@ -168,22 +235,15 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
     int np = 0;
     BKR_TRY(apply_M(ctx, mass, N, BKR_F64, Xcur, w->R64, gate));
     BKR_TRY(launch_axpby(ctx, n, BKR_F64, 1.0, w->Bn, -1.0, w->R64, w->R64, gate));
-    BKR_TRY(launch_gram_partials(ctx, N, BKR_F64, w->R64, w->R64, 1, &np, gate));
+    BKR_TRY(blk_gram(ctx, N, BKR_F64, w->R64, w->R64, &np, gate));
     BKR_TRY(launch_small(ctx, small_args(w, small_mode, np, tol, delta, mixed, ctx)));
     // Q = R C^-1 (Alg. 2 l.4), stored in the inner precision
-    BKR_TRY(launch_block_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr, 1)); // C^-1 upper triangular
-    if (fuse_q(N)) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
+    BKR_TRY(blk_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr, 1)); // C^-1 upper triangular
+    if (fuse_qpx(ctx, N)) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
         set_identity_kernel<<<1, 256, 0, ctx->stream>>>(N, w->Sinv);
         BKR_TRY(bkr_check_launch(ctx));
     }
     return BKR_OK;
-}
-
-// BKR_NO_DEFER=1 (comparison runs): X update as its own kernel right after l.9, as in the unfused Algorithm 1
-static bool defer_x(int N)
-{
-    static const bool d = getenv("BKR_NO_DEFER") == nullptr;
-    return d && N <= FUSE_MAX_N;
 }
 
 // flags as the loop expects them after (re)initialisation: nothing pending for X
@@ -198,7 +258,7 @@ static int reset_flags(bkr_ctx *ctx, Workspace *w)
 // reliable update)
 static int flush_x(bkr_ctx *ctx, Workspace *w)
 {
-    if (!defer_x(w->N)) return BKR_OK;
+    if (!fuse_qpx(ctx, w->N)) return BKR_OK;
     BKR_TRY(launch_block_update(ctx, w->N, BKR_F64, w->prec, w->W, w->Xn, w->P, w->Xn, &w->flags->xidle));
     BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xpend, 0, sizeof(int), ctx->stream));
     BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xidle, 1, sizeof(int), ctx->stream));
@@ -212,37 +272,36 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     const int *done = &w->flags->done;
     int np = 0;
     void *t;
-    const bool defer = defer_x(N);
-    if (defer) {
-        // l.8  P = Q + P S^dag, fused with l.10 of the PREVIOUS iteration, X += P_old (beta C)_old: one pass over P for
-        // both (the deferral of PAPER.md:243).  flags->xpend says whether a W is waiting; flush_x() applies the last one.
-        // With fuse_q(N) also Alg. 2 l.4 of the previous iteration, Q = Q' S^-1, in the same pass (Q' is read anyway).
-        if (fuse_q(N)) BKR_TRY(launch_pqx_update(ctx, N, pr, w->Sinv, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
-        else BKR_TRY(launch_px_update(ctx, N, pr, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
+    const bool fused = fuse_qpx(ctx, N);
+    if (fused) {
+        // l.8  P = Q + P S^dag, fused with Alg. 2 l.4 of the PREVIOUS iteration (Q = Q' S^-1: Q' is read anyway) and with its
+        // l.10, X += P_old (beta C)_old: one pass over Q, P, X (the deferral of PAPER.md:243).  flags->xpend says whether
+        // a W is waiting; flush_x() applies the last one.
+        BKR_TRY(launch_pqx_update(ctx, N, pr, w->Sinv, w->Sdag, w->W, w->Q, w->P, w->P2, w->Xn, w->flags));
     } else {
-        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done, 2)); // S^dag lower triangular
+        BKR_TRY(blk_update(ctx, N, pr, pr, w->Sdag, w->Q, w->P, w->P2, done, 2)); // S^dag lower triangular
     }
     t = w->P; w->P = w->P2; w->P2 = t;
     // l.9  beta = (P^dag M P)^-1 ; W = beta C
     BKR_TRY(apply_M(ctx, mass, N, pr, w->P, w->AP, done));
-    BKR_TRY(launch_gram_partials(ctx, N, pr, w->P, w->AP, 1, &np, done));
+    BKR_TRY(blk_gram(ctx, N, pr, w->P, w->AP, &np, done));
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_BETA, np, tol, delta, mixed, ctx)));
     // l.10 X = X + P (beta C)     (X in fp64 also in the mixed solver): deferred, see above
-    if (!defer) BKR_TRY(launch_block_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done));
+    if (!fused) BKR_TRY(blk_update(ctx, N, BKR_F64, pr, w->W, w->Xn, w->P, w->Xn, done, 0));
     // l.11 Q S = Q - (M P) beta   (thin QR = Gram + Cholesky + scale, Algorithm 2)
-    static const bool fuse_gram = getenv("BKR_NO_GRAMFUSE") == nullptr;
+    const bool fuse_gram = !(ctx->ablation & (BKR_ABL_UNFUSED_GRAM | BKR_ABL_VECTOR_BLAS));
     // N <= 16 only: with 3-4 column tiles the reduction's 6-10 tile-pair accumulators no longer fit beside the update's
     // (ptxas spills; measured 4.08 vs 3.76 ms per iteration at N = 24, 5.76 vs 5.58 at N = 32 on 32^4)
     if (fuse_gram && N <= 16) { // one pass: Q' and stage 1 of H = Q'^dag Q'
         BKR_TRY(launch_update_gram(ctx, N, pr, w->negbeta, w->Q, w->AP, w->Q, &np, done));
     } else {
-        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done));
-        BKR_TRY(launch_gram_partials(ctx, N, pr, w->Q, w->Q, 1, &np, done));
+        BKR_TRY(blk_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done, 0));
+        BKR_TRY(blk_gram(ctx, N, pr, w->Q, w->Q, &np, done));
     }
     // l.12 C = S C, residual norms, convergence / reliable-update flags
     BKR_TRY(launch_small(ctx, small_args(w, SMALL_QR, np, tol, delta, mixed, ctx)));
-    if (!fuse_q(N)) {
-        BKR_TRY(launch_block_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done, 1)); // S^-1 upper triangular
+    if (!fused) {
+        BKR_TRY(blk_update(ctx, N, pr, pr, w->Sinv, nullptr, w->Q, w->Q2, done, 1)); // S^-1 upper triangular
         t = w->Q; w->Q = w->Q2; w->Q2 = t;
     }
     return BKR_OK;

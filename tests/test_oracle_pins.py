@@ -236,3 +236,36 @@ def test_mixed_precision_reliable_updates_reach_true_tolerance(cfg1):
     assert oracle.true_relres(D4, fat, lng, 0.1, B, mix["X"]).max() <= 1e-10
     assert mix["iters"] <= 2 * pure["iters"]
     assert H.relerr_inf(mix["X"], pure["X"]) < 1e-8
+
+
+def test_U13_fp32_storage_stalls_true_residual_without_updates(cfg1):
+    """The oracle's fp32 emulation (round_f32 on P, Q, MP and the inner links, U13) must bite: with the delta trigger
+    switched off (delta = 1e-30) the first reliable update only happens when the ITERATED residual reports tol, and the
+    true residual that update computes is stuck near fp32 precision (SURVEY U13 probe: ~1e-7 .. 1e-6), orders of
+    magnitude above the 1e-10 the iteration claims; the solve then stalls there (the search space was not preserved).
+    With round_f32 a no-op the jump would not exist and that one update would end the solve.  The same solve with
+    delta = 0.1 reaches the true 1e-10."""
+    fat, lng, B = cfg1
+    tol = 1e-10
+    lazy = oracle.block_cg(D4, fat, lng, 0.1, B, tol=tol, mixed=True, delta=1e-30, maxiter=400)
+    hist = lazy["hist"]
+    first = next(i for i in range(1, len(hist)) if hist[i] > 20 * hist[i - 1])  # the update replaces r by the true value
+    assert hist[first - 1] < 1e-8 and hist[first - 1] > tol * 0.01  # the iteration had (nearly) reported convergence ...
+    assert 1e-9 < hist[first] < 1e-5                                 # ... while the true residual sat at fp32 level
+    assert lazy["status"] == -6 and lazy["reliable_updates"] == 1 and hist[-1] > 1e-8  # and it never recovers
+    mix = oracle.block_cg(D4, fat, lng, 0.1, B, tol=tol, mixed=True, delta=0.1)
+    assert mix["status"] == 0 and oracle.true_relres(D4, fat, lng, 0.1, B, mix["X"]).max() <= tol
+
+
+def test_P8_Qold_dag_P_is_identity_after_line8(cfg1):
+    """(Q_old)^dag P = 1 right after Alg. 1 l.8 -- the new residual block is orthogonal to the previous
+    search directions -- in pure fp64 and across block reliable updates (S = C_new C_prev^-1, U12, is what keeps it)."""
+    fat, lng, B = cfg1
+    N = B.shape[0]
+    pure = oracle.block_cg(D4, fat, lng, 0.1, B, tol=1e-10, ntrace=40)
+    for k in range(40):
+        assert np.abs(pure["QP"][k] - np.eye(N)).max() <= 1e-9, k
+    mix = oracle.block_cg(D4, fat, lng, 0.1, B, tol=1e-10, mixed=True, delta=0.1, ntrace=60)
+    assert mix["reliable_updates"] >= 3
+    for k in range(60):
+        assert np.abs(mix["QP"][k] - np.eye(N)).max() <= 2e-5, k  # fp32 storage of P and Q
