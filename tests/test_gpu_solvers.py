@@ -212,3 +212,57 @@ def test_config2_mixed_precision(cfg2):
     X, rr, st = ctx.solve_block(0.05, torch.from_numpy(B).cuda(), tol=TOL, inner_prec=binding.F32, delta=0.1)
     assert st["status"] == binding.OK and st["reliable_updates"] >= 3
     assert oracle.true_relres(dims, fat, lng, 0.05, B, X.cpu().numpy()).max() <= TOL
+
+
+# ------------------------------------------------------------------ blocks of more than 16 rhs (host control flow of solver.cu)
+
+@pytest.fixture(scope="module")
+def lat8():
+    dims = (8, 8, 8, 8)
+    fat, lng = H.np_links(dims, "perturbed", seed=71)
+    return dims, fat, lng, _ctx(dims, fat, lng)
+
+
+@pytest.mark.parametrize("N", [20, 24, 28, 32])
+def test_large_block_solve_vs_oracle(lat8, N):
+    """N = 17..24: fused Q/P/X update without Gram fusion; N > 24: the unfused path with per-iteration Q/Q2 and P/P2
+    pointer swaps and tri = 1/2 block updates.  Solution, true residual and iteration count against
+    the oracle's blockCGrQ; the k-th iterate (maxiter = k) must match too."""
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, ctx = lat8
+    B = H.np_sources(dims, N, seed=72 + N)
+    Bd = torch.from_numpy(B).cuda()
+    X, rr, st = ctx.solve_block(0.05, Bd, tol=TOL)
+    assert st["status"] == binding.OK and max(rr) <= TOL
+    ro = oracle.block_cg(dims, fat, lng, 0.05, B, tol=TOL)
+    assert ro["status"] == 0
+    assert _soldiff(X.cpu().numpy(), ro["X"]) <= 1e-8
+    assert abs(st["iters"] - ro["iters"]) <= 3
+    assert oracle.true_relres(dims, fat, lng, 0.05, B, X.cpu().numpy()).max() <= TOL
+    for k in (1, 4):
+        Xk, _, stk = ctx.solve_block(0.05, Bd, tol=TOL, maxiter=k)
+        assert stk["iters"] == k
+        assert _soldiff(Xk.cpu().numpy(), oracle.block_cg(dims, fat, lng, 0.05, B, tol=TOL, maxiter=k)["X"]) <= 1e-10
+
+
+@pytest.mark.parametrize("N", [24, 32])
+def test_large_block_mixed_precision(lat8, N):
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, ctx = lat8
+    B = H.np_sources(dims, N, seed=82 + N)
+    X, rr, st = ctx.solve_block(0.05, torch.from_numpy(B).cuda(), tol=TOL, inner_prec=binding.F32, delta=0.1)
+    assert st["status"] == binding.OK and st["reliable_updates"] >= 3
+    assert oracle.true_relres(dims, fat, lng, 0.05, B, X.cpu().numpy()).max() <= TOL
+    ro = oracle.block_cg(dims, fat, lng, 0.05, B, tol=TOL)
+    assert _soldiff(X.cpu().numpy(), ro["X"]) <= 1e-8
+
+
+def test_duplicate_rhs_reports_breakdown_mixed(cfg1):
+    """the same negative case with the fp32 inner solver: the rank deficit is caught by the fp64 QR of the initial
+    residual (Alg. 1 l.4 runs in fp64 also in the mixed solver), before any fp32 Gram matrix is factored"""
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, B, ctx = cfg1
+    B2 = B.copy()
+    B2[3] = B2[0]
+    _, _, st = ctx.solve_block(0.1, torch.from_numpy(B2).cuda(), tol=TOL, inner_prec=binding.F32, delta=0.1)
+    assert st["status"] == binding.EBREAKDOWN
