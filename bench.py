@@ -2,7 +2,7 @@
 """bench.py -- measurement harness.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl bkr|reference] [--workload cfg3|cfg4|cfg5|cfg2]
-                    [--no-solve] [--sweep]
+                    [--no-solve] [--sweep] [--microbench] [--ablation]
 
 A "step" is one blockCGrQ iteration (Algorithm 1 l.8-l.12 of arXiv:1710.09745: 2 multi-rhs Dslash, 2 Gram
 reductions, the block updates of P, X, Q and the one-CTA small-matrix kernels) on the workload's block of N rhs,
@@ -153,15 +153,57 @@ def time_loop(torch, fn, reps, warmup):
 
 SM_COUNT, SM_MAX_MHZ = 148, 1965.0
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed `ncu --set full`
-# capture of this same bench command (profiles/r1_ncu_summary.md); None where no capture exists.
-NCU_TRAFFIC = {("cfg3", 16, "f64"): 4.501845e9 + 0.788309e9}
+
+def kernel_source_hash():
+    """sha256 over the CUDA sources of the library: the key a stored ncu capture is valid for."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_1710_09745_b200", "csrc", "*.cu*"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()
+
+
+def ncu_traffic(workload, N, dtype):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
+    capture (profiles/r2_traffic.json).  The capture names the sha256 of the kernel sources it was taken from; if the
+    sources have changed since, the number is stale and None is returned instead (never a pasted literal)."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    d = json.load(open(path))
+    for e in d.get("captures", []):
+        if e["workload"] == workload and e["N"] == N and e["dtype"] == dtype:
+            info = {"commit": e.get("commit"), "source_sha256": e.get("source_sha256"), "kernel": e.get("kernel")}
+            if e.get("source_sha256") == kernel_source_hash():
+                return e["dram_bytes_read"] + e["dram_bytes_write"], info
+            info["stale"] = True
+            return None, info
+    return None, None
+
+
+# FMA-pipe peaks (GFLOP/s).  Default: DESIGN.md section 6.4's derivation from the guide's unit counts (148 SMs x 64 FP64 /
+# 128 FP32 lanes x 2 flop x 1.965 GHz); run_bkr() replaces them by the register-only microbenchmark of bkr_microbench
+# measured on this box (SURVEY.md section 7.2-1) and says so in the JSON line.
+ALU_PEAK = {True: SM_COUNT * 64 * 2 * SM_MAX_MHZ * 1e-3, False: SM_COUNT * 128 * 2 * SM_MAX_MHZ * 1e-3, "source": "derived (unit counts x 1.965 GHz)"}
+
+MICROBENCH_KINDS = [(0, "fp64_fma_tflops", 1e-9), (1, "fp32_fma_tflops", 1e-9), (2, "fp64_mma_m8n8k4_tflops", 1e-9),
+                    (6, "stencil_fma_pattern_rhs_major_tflops", 1e-9), (7, "stencil_fma_pattern_link_major_tflops", 1e-9),
+                    (3, "l2_to_sm_ldg_tbps", 1e-9), (4, "l2_to_sm_tma_tbps", 1e-9), (5, "smem_read_tbps", 1e-9)]
+
+
+def run_microbench(ctx, reps=5):
+    """on-chip peaks measured on this box (bkr_microbench): units / ms * 1e-9 = TFLOP/s or TB/s"""
+    out = {}
+    for kind, name, scale in MICROBENCH_KINDS:
+        ms, units = ctx.microbench(kind, reps)
+        out[name] = units / ms * scale
+    return out
 
 
 def alu_peak_gflops(fp64):
-    """FMA-pipe peak DESIGN.md section 6.4 derives from the guide's unit counts: 148 SMs x 64 FP64 (128 FP32) lanes x
-    2 flop x 1.965 GHz.  The DMMA path of the multi-BLAS kernels has the same FP64 peak (measured 36.8 TFLOP/s)."""
-    return SM_COUNT * (64 if fp64 else 128) * 2 * SM_MAX_MHZ * 1e-3
+    return ALU_PEAK[bool(fp64)]
 
 
 def roofline_entry(ms, by, fl, hbm, fp64_math):
@@ -197,6 +239,13 @@ def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
     out["dslash"]["variant"] = {0: "dslash_kernel (register tiling + link ring)",
                                 1: "dslash_win_kernel (shared-memory window, cluster-multicast links)"}.get(ctx.dslash_variant(), "?")
 
+    def f_dslash_xpay():
+        s, d = rot()
+        ctx.dslash_xpay(i[0] & 1, N, 4e-4, blk[nb], s, d, prec)
+    ms = time_loop(torch, f_dslash_xpay, reps, warmup)
+    by, fl = bytes_dslash(dims, N, w, xpay=True), flops_dslash(dims, N, xpay=True)
+    out["dslash_xpay"] = roofline_entry(ms, by, fl, hbm, prec == binding.F64)
+
     def f_gram2():
         s, d = rot()
         ctx.gram(N, s, d, hermitian=False, prec=prec, out=K)
@@ -224,6 +273,24 @@ def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
     ms = time_loop(torch, f_axpy, reps, warmup)
     by, fl = 3 * block_bytes(dims, N, w), 8 * L * N * N
     out["block_axpy"] = roofline_entry(ms, by, fl, hbm, True)
+
+    # the two fused kernels of the iteration: 6 and 3 block passes
+    tri_u = torch.triu(a).contiguous()
+    tri_l = torch.tril(a).contiguous()
+    X64 = blk[nb] if prec == binding.F64 else ctx.empty_native(N, binding.F64).normal_()
+
+    def f_pqx():
+        s, d = rot()
+        ctx.block_qpx_update(N, tri_u, tri_l, a, s, d, blk[(i[0] + 2) % nb], X64, prec)
+    ms = time_loop(torch, f_pqx, reps, warmup)
+    by = 4 * block_bytes(dims, N, w) + 2 * block_bytes(dims, N, 8)  # Q', P in, Q, P out (storage precision); X in and out (fp64)
+    out["pqx_update"] = roofline_entry(ms, by, 16 * L * N * N, hbm, True)  # ~ half of 3 x 8 L N^2 for the triangular pair
+
+    def f_ug():
+        s, d = rot()
+        ctx.block_axpy_gram(N, a, s, d, prec, out=K)
+    ms = time_loop(torch, f_ug, reps, warmup)
+    out["update_gram"] = roofline_entry(ms, 3 * block_bytes(dims, N, w), 8 * L * N * N + 4 * L * N * (N + 1), hbm, True)
     return out
 
 
@@ -232,15 +299,28 @@ def kernel_numbers(torch, ctx, binding, dims, N, prec, reps, warmup, hbm):
 _ORACLE_INPUTS = {}
 
 
-def oracle_sample(dims_full, N, kind, seed=5):
-    """One blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update) with the oracle on a bounded
-    sample: the same N and link generator on a lattice shrunk until it is ~10-30 s of CPU work.
+def _omp_set_threads(n):
+    """thread count of the oracle's OpenMP loops (same libgomp instance as liboracle.so)"""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except OSError:
+        return False
+
+
+def oracle_sample(dims_full, N, kind, seed=5, max_sites_rhs=None, threads=None):
+    """One blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update) with the oracle, as it stands, on the host
+    cores.  Default: the FULL lattice of the workload when that is at most configs[2]'s size (32^3 x 64 x 16 rhs: a few
+    seconds on 16 cores); larger workloads and the 1-thread figure use the same N and link generator on a lattice halved
+    along its longest directions until it is bounded (stated in the returned description).
     returns (seconds, algorithmic bytes of the sample, sample description, threads)."""
     import numpy as np
     import oracle
     from paper_1710_09745_b200 import synth
     dims = list(dims_full)
-    while volume(dims) * N > 32 ** 4 * 16:  # ~4 s on 8 cores = about 30 s of CPU work
+    cap = max_sites_rhs if max_sites_rhs else 32 ** 3 * 64 * 16
+    while volume(dims) * N > cap:
         k = max(range(4), key=lambda mu: dims[mu])
         dims[k] //= 2
     dims = tuple(dims)
@@ -254,6 +334,10 @@ def oracle_sample(dims_full, N, kind, seed=5):
     Q = Q.copy()
     a = (np.eye(N) * 0.5).astype(np.complex128)
     oracle.lib()
+    ncpu = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    used = ncpu
+    if threads is not None and _omp_set_threads(threads):
+        used = threads
     t0 = time.perf_counter()
     AP = oracle.apply_M(dims, fat, lng, 0.05, P)
     oracle.gram(P, AP)
@@ -261,10 +345,12 @@ def oracle_sample(dims_full, N, kind, seed=5):
     for _ in range(4):
         oracle.block_axpy(a, P, Q)
     dt = time.perf_counter() - t0
-    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
-    desc = "one blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update), N=%d, on a %s lattice" % (
-        N, "x".join(str(d) for d in dims))
-    return dt, bytes_iteration(dims, N, 8), desc, threads
+    if threads is not None:
+        _omp_set_threads(ncpu)
+    full = tuple(dims) == tuple(dims_full)
+    desc = "one blockCGrQ iteration's operations (1 x M, 2 x Gram, 4 x block update), N=%d, on %s %s lattice" % (
+        N, "the full" if full else "a reduced", "x".join(str(d) for d in dims))
+    return dt, bytes_iteration(dims, N, 8), desc, used
 
 
 def run_reference(args):
@@ -344,6 +430,10 @@ def run_bkr(args):
     ctx.load_links(fat, lng, also_f32=True)
     del fat, lng
     torch.cuda.empty_cache()
+    # on-chip peaks measured on this box: the "alu" roofline denominators
+    micro = run_microbench(ctx)
+    ALU_PEAK[True], ALU_PEAK[False] = micro["fp64_fma_tflops"] * 1e3, micro["fp32_fma_tflops"] * 1e3
+    ALU_PEAK["source"] = "measured (bkr_microbench register-only FMA, this run)"
     sampler = ClockSampler(local)
     sampler.start()  # nvidia-smi takes a while to start: launched before the warm-up, windowed to the timed region
 
@@ -363,6 +453,11 @@ def run_bkr(args):
         dist.barrier()
     ms_total = max_over_ranks(dist, e0.elapsed_time(e1), dev)
     ms_step = ms_total / args.steps
+    # every timed iteration must have done its full work: the loop kernels become no-ops once the device-side `done`
+    # flag is set (convergence or a Cholesky breakdown), which would time empty launches
+    state = ctx.solver_state()
+    if state["done"] or state["breakdown"] or state["iters"] != args.warmup + args.steps:
+        raise RuntimeError("timed iterations did not all run: %r (expected %d iterations)" % (state, args.warmup + args.steps))
     by_iter = bytes_iteration(dims, N, w)
     value = replicas_value(world, by_iter, ms_step)
 
@@ -408,8 +503,15 @@ def run_bkr(args):
         dt, sby, desc, threads = oracle_sample(dims, N, kind)
         cpu = {"value": sby / dt * 1e-9, "unit": "GB/s", "cores": threads, "kind": "oracle", "sample": desc,
                "seconds": dt}
+        dt1, sby1, desc1, th1 = oracle_sample(dims, N, kind, max_sites_rhs=16 ** 3 * 32 * 16, threads=1)
+        cpu["one_thread"] = {"value": sby1 / dt1 * 1e-9, "unit": "GB/s", "cores": th1, "sample": desc1, "seconds": dt1}
+
+    ablation = None
+    if rank == 0 and world == 1 and args.ablation:
+        ablation = run_ablation(torch, ctx, binding, mass, B, prec)
 
     d = kern["dslash"]
+    traffic, traffic_info = ncu_traffic(args.workload, N, "f64" if prec == binding.F64 else "f32")
     line = {
         "metric": "blockcg_iteration_effective_GBps", "value": value, "unit": "GB/s", "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
@@ -423,21 +525,55 @@ def run_bkr(args):
         "GFLOPS_iteration": world * flops_iteration(dims, N) / ms_step * 1e-6,
         "roofline": {"bound": "hbm", "kernel": "%s: multi-rhs Dslash, one parity, N=%d" % (d.get("variant", "dslash"), N),
                      "achieved": d["GBps"], "peak": hbm, "unit": "GB/s", "frac": d["GBps"] / hbm,
-                     "traffic": NCU_TRAFFIC.get((args.workload, N, "f64" if prec == binding.F64 else "f32")),
+                     "traffic": traffic, "traffic_capture": traffic_info,
                      "frac_roofline": d["frac_roofline"], "binding": d["binding"],
                      "peak_source": peak_src, "ms_per_launch": d["ms"],
                      "algorithmic_bytes_per_launch": bytes_dslash(dims, N, w), "GFLOPS": d["GFLOPS"]},
         "kernels": kern,
+        "alu_peak": {"fp64_gflops": ALU_PEAK[True], "fp32_gflops": ALU_PEAK[False], "source": ALU_PEAK["source"]},
+        "microbench": micro,
+        "iterations_completed": state["iters"],
         "e2e": e2e,
         "gpu_launches": launches,
         "clocks": clocks,
         "cpu_baseline": cpu,
         "solve": solve,
+        "ablation": ablation,
     }
     print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
     return 0
+
+
+def run_ablation(torch, ctx, binding, mass, B, prec, iters=100):
+    """The comparison of the paper's Fig. 4: time for 100 blockCGrQ iterations with (i) nothing
+    blocked -- single-vector caxpys / dot products and one stencil call per rhs, (ii) block BLAS only, (iii) block BLAS +
+    block Dslash (unfused kernels), (iv) the shipped iteration (fused updates, deferred X).  Same arithmetic in every arm
+    (tests/test_gpu_multiblas_instances.py::test_ablation_switches...)."""
+    arms = [("no_block", binding.ABL_VECTOR_BLAS | binding.ABL_VECTOR_DSLASH | binding.ABL_UNFUSED_UPDATES | binding.ABL_UNFUSED_GRAM),
+            ("block_blas", binding.ABL_VECTOR_DSLASH | binding.ABL_UNFUSED_UPDATES | binding.ABL_UNFUSED_GRAM),
+            ("block_blas_block_dslash", binding.ABL_UNFUSED_UPDATES | binding.ABL_UNFUSED_GRAM),
+            ("fused (shipped)", 0)]
+    out = {"iterations": iters, "N": int(B.shape[0])}
+    try:
+        for name, mask in arms:
+            ctx.set_option(binding.OPT_ABLATION, mask)
+            ctx.solve_block(mass, B, tol=1e-10, maxiter=0, inner_prec=prec)  # re-initialises the solver state
+            ctx.bench_iterations(mass, B, 2, prec)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            n = ctx.bench_iterations(mass, B, iters, prec)
+            e1.record()
+            torch.cuda.synchronize()
+            st = ctx.solver_state()
+            out[name] = {"seconds": e0.elapsed_time(e1) * 1e-3, "launches": n, "completed": st["iters"], "done": st["done"]}
+    finally:
+        ctx.set_option(binding.OPT_ABLATION, 0)
+        ctx.solve_block(mass, B, tol=1e-10, maxiter=0, inner_prec=prec)
+    out["paper_context"] = "paper Fig. 4 (GP100, fp64): with block BLAS + block Dslash the time per rhs is about half that of 1-rhs CG"
+    return out
 
 
 def solve_comparison(torch, ctx, binding, mass, B, args):
@@ -495,6 +631,8 @@ def main():
     ap.add_argument("--no-solve", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--sweep", action="store_true")
+    ap.add_argument("--microbench", action="store_true", help="print the on-chip microbenchmark numbers only")
+    ap.add_argument("--ablation", action="store_true", help="add the Fig. 4-style ablation (100 iterations per arm)")
     ap.add_argument("--maxiter", type=int, default=20000)
     ap.add_argument("--cg-rhs", type=int, default=2, help="sequential CG is measured on this many rhs and scaled to N")
     args = ap.parse_args()
@@ -503,6 +641,10 @@ def main():
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.microbench:
+        from paper_1710_09745_b200 import binding
+        print(json.dumps({"microbench": run_microbench(binding.Context((8, 8, 8, 8)), reps=10), "unit": "TFLOP/s or TB/s"}))
+        return 0
     return run_bkr(args)
 
 

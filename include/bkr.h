@@ -93,6 +93,11 @@ int bkr_unpack(bkr_ctx *ctx, int N, int prec, const void *native, void *canonica
  * out_parity 1: odd <- even (D_oe); 0: even <- odd (D_eo). */
 int bkr_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out);
 
+/* The stencil with its "xpay" epilogue, the second half of M (the 1158 flop per site include the 12
+ * of this axpy): out = a * xp - D_{out_parity, 1-out_parity} in.  xp, out: native blocks on parity out_parity; in on the
+ * other parity; out must alias neither. */
+int bkr_dslash_xpay(bkr_ctx *ctx, int out_parity, int N, int prec, double a, const void *xp, const void *in, void *out);
+
 /* out = 4 m^2 in - D_eo (D_oe in) on even sites ("Schur decomposed"); in/out native. */
 int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out);
 
@@ -163,6 +168,12 @@ int bkr_solve_cg_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void
  * in *launches (HOST, may be NULL). */
 int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void *B, int iters,
                          long long *launches);
+
+/* Device-side loop state after bkr_bench_iterations (or a solve), read back with a stream synchronisation:
+ * state[0] = iterations completed since the last (re)initialisation, state[1] = done flag (1: the loop kernels have
+ * become no-ops), state[2] = Cholesky breakdown, state[3] = an X update is still deferred.  state: HOST, 4 ints.
+ * bench.py uses it to prove that every timed iteration did its full work.  BKR_EINVAL before the first solve. */
+int bkr_solver_state(bkr_ctx *ctx, int *state);
 
 /* Which stencil kernel the most recent Dslash launch of this context used (bkr_dslash, bkr_apply_M or inside a solver):
  * 0 = plain multi-rhs kernel (register tiling + link ring), 2 = row-window kernel, 1 = shared-memory window kernel with

@@ -20,10 +20,10 @@ OPT_L2_BUDGET_MB, OPT_ROW_UNIT_TILES, OPT_ROW_VEC_POLICY, OPT_ABLATION = 0, 1, 2
 ABL_UNFUSED_UPDATES, ABL_UNFUSED_GRAM, ABL_VECTOR_BLAS, ABL_VECTOR_DSLASH = 1, 2, 4, 8
 
 SYMBOLS = (
-    "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash",
+    "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash", "bkr_dslash_xpay",
     "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_update", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
-    "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench",
+    "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench", "bkr_solver_state",
 )
 
 
@@ -64,6 +64,7 @@ def lib():
             "bkr_pack": (ci, [vp, ci, ci, vp, vp]),
             "bkr_unpack": (ci, [vp, ci, ci, vp, vp]),
             "bkr_dslash": (ci, [vp, ci, ci, ci, vp, vp]),
+            "bkr_dslash_xpay": (ci, [vp, ci, ci, ci, cd, vp, vp, vp]),
             "bkr_apply_M": (ci, [vp, cd, ci, ci, vp, vp]),
             "bkr_gram": (ci, [vp, ci, ci, vp, vp, ci, vp]),
             "bkr_block_axpy": (ci, [vp, ci, ci, vp, vp, vp]),
@@ -83,6 +84,7 @@ def lib():
             "bkr_dslash_variant": (ci, [vp]),
             "bkr_set_dslash_variant": (ci, [vp, ci]),
             "bkr_set_option": (ci, [vp, ci, ci]),
+            "bkr_solver_state": (ci, [vp, ctypes.POINTER(ci)]),
             "bkr_microbench": (ci, [vp, ci, ci, ctypes.POINTER(cd)]),
         }
         for name, (res, args) in sig.items():
@@ -174,6 +176,12 @@ class Context:
     def dslash(self, out_parity, N, src, dst, prec=F64):
         self._check(lib().bkr_dslash(self._h, int(out_parity), int(N), int(prec), _dev_ptr(src, "in"), _dev_ptr(dst, "out")),
                     "bkr_dslash")
+        return dst
+
+    def dslash_xpay(self, out_parity, N, a, xp, src, dst, prec=F64):
+        """dst = a * xp - D src (the second half of M, bkr.h)."""
+        self._check(lib().bkr_dslash_xpay(self._h, int(out_parity), int(N), int(prec), float(a), _dev_ptr(xp, "xp"),
+                                          _dev_ptr(src, "in"), _dev_ptr(dst, "out")), "bkr_dslash_xpay")
         return dst
 
     def apply_M(self, mass, N, src, dst, prec=F64):
@@ -300,6 +308,12 @@ class Context:
         self._check(lib().bkr_bench_iterations(self._h, float(mass), N, int(prec), _dev_ptr(B, "B"), int(iters),
                                                ctypes.byref(n)), "bkr_bench_iterations")
         return int(n.value)
+
+    def solver_state(self):
+        """dict(iters, done, breakdown, xpend) of the device-side loop flags (bkr.h)."""
+        st = (ctypes.c_int * 4)()
+        self._check(lib().bkr_solver_state(self._h, st), "bkr_solver_state")
+        return {"iters": st[0], "done": st[1], "breakdown": st[2], "xpend": st[3]}
 
     def microbench(self, kind, reps=5):
         """(ms per launch, flop or bytes per launch) of the on-chip microbenchmark `kind` (bkr.h)."""

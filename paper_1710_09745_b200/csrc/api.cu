@@ -107,6 +107,14 @@ int bkr_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, vo
     return launch_dslash(ctx, out_parity, N, prec, in, out, nullptr, 0.0, nullptr);
 }
 
+int bkr_dslash_xpay(bkr_ctx *ctx, int out_parity, int N, int prec, double a, const void *xp, const void *in, void *out)
+{
+    if (!ctx || !valid_n(N) || !valid_prec(prec) || !in || !out || !xp || in == out || xp == out) return BKR_EINVAL;
+    if (out_parity != 0 && out_parity != 1) return BKR_EINVAL;
+    BKR_ENTER(ctx);
+    return launch_dslash(ctx, out_parity, N, prec, in, out, xp, a, nullptr);
+}
+
 int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void *out)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !in || !out || in == out) return BKR_EINVAL;
@@ -292,6 +300,13 @@ int bkr_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const void 
     BKR_ENTER(ctx);
     if (!ctx->links64 || (prec == BKR_F32 && !ctx->links32)) return BKR_ENOLINKS;
     return solver_bench_iterations(ctx, mass, N, prec, (const double2 *)B, iters, launches);
+}
+
+int bkr_solver_state(bkr_ctx *ctx, int *state)
+{
+    if (!ctx || !state) return BKR_EINVAL;
+    BKR_ENTER(ctx);
+    return solver_read_flags(ctx, state);
 }
 
 int bkr_microbench(bkr_ctx *ctx, int kind, int reps, double *result)

@@ -209,6 +209,7 @@ int solver_cg(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, do
               int batched, int *iters, double *true_relres, bkr_stats *stats);
 int solver_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const double2 *B, int iters,
                             long long *launches);
+int solver_read_flags(bkr_ctx *ctx, int out[4]);
 void solver_free_workspace(bkr_ctx *ctx);
 void solver_invalidate(bkr_ctx *ctx); // links changed: cached bench state is stale
 int ensure_partials(bkr_ctx *ctx, size_t bytes);

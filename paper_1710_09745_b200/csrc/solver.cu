@@ -519,3 +519,15 @@ int solver_bench_iterations(bkr_ctx *ctx, double mass, int N, int prec, const do
     if (launches) *launches = ctx->launches - l0;
     return BKR_OK;
 }
+
+int solver_read_flags(bkr_ctx *ctx, int out[4])
+{
+    Workspace *w = ctx->ws;
+    if (!w || !w->flags) return BKR_EINVAL;
+    BKR_TRY(read_flags(ctx, w));
+    out[0] = w->h_flags->iters;
+    out[1] = w->h_flags->done;
+    out[2] = w->h_flags->breakdown;
+    out[3] = w->h_flags->xpend;
+    return BKR_OK;
+}
