@@ -194,8 +194,16 @@ int bkr_set_dslash_variant(bkr_ctx *ctx, int variant);
  *   BKR_OPT_ROW_VEC_POLICY  L2 eviction priority of its z/t neighbour loads: 0 evict_normal, 1 evict_last
  *   BKR_OPT_ABLATION        bit mask of BKR_ABL_*: parts of the method switched off for the comparison of the paper's
  *                           Fig. 4 (no block / block BLAS / block BLAS + block Dslash).  Results are
- *                           the same up to rounding; only the kernels that produce them change.  0 = the full method. */
-enum { BKR_OPT_L2_BUDGET_MB = 0, BKR_OPT_ROW_UNIT_TILES = 1, BKR_OPT_ROW_VEC_POLICY = 2, BKR_OPT_ABLATION = 3 };
+ *                           the same up to rounding; only the kernels that produce them change.  0 = the full method.
+ *   BKR_OPT_TUNE + k        stencil launch parameter k of BKR_TUNE_* below (ring depths, segment length, thread
+ *                           shape); every setting computes the same result. */
+enum { BKR_OPT_L2_BUDGET_MB = 0, BKR_OPT_ROW_UNIT_TILES = 1, BKR_OPT_ROW_VEC_POLICY = 2, BKR_OPT_ABLATION = 3, BKR_OPT_TUNE = 16 };
+enum {
+    BKR_TUNE_WIN_STAGES = 0,      /* window stencil: hop-stage ring depth, 2-8 (default: the deepest that fits)          */
+    BKR_TUNE_WIN_SEGLEN = 2,      /* 64-site tiles per segment (default 8)                                                */
+    BKR_TUNE_WIN_SLIM = 3,        /* 2 = keep spare window slots instead of releasing the lower halo early                */
+    BKR_TUNE_COUNT = 16
+};
 enum {
     BKR_ABL_UNFUSED_UPDATES = 1, /* Q, P, X updates as separate kernels, X updated right after Alg. 1 l.9 (no deferral)   */
     BKR_ABL_UNFUSED_GRAM = 2,    /* Q' = Q - MP beta and its Gram matrix as two kernels                                  */

@@ -342,7 +342,9 @@ int bkr_set_option(bkr_ctx *ctx, int option, int value)
     case BKR_OPT_ROW_UNIT_TILES: ctx->row_unit_tiles = value; break;
     case BKR_OPT_ROW_VEC_POLICY: ctx->row_vec_policy = value; break;
     case BKR_OPT_ABLATION: ctx->ablation = value & 15; break;
-    default: return BKR_EINVAL;
+    default:
+        if (option < BKR_OPT_TUNE || option >= BKR_OPT_TUNE + BKR_TUNE_COUNT) return BKR_EINVAL;
+        ctx->tune[option - BKR_OPT_TUNE] = value;
     }
     // blocking tables are rebuilt on the next stencil call
     ctx->tile_order_key = ctx->win_key = ctx->row_key = -1;

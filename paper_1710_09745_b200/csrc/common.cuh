@@ -66,6 +66,7 @@ struct bkr_ctx {
     int dslash_force; // bkr_set_dslash_variant: -1 automatic, 0 plain, 1 window, 2 row window
     int l2_budget_mb, row_unit_tiles, row_vec_policy; // bkr_set_option (0 = built-in default)
     int ablation;       // BKR_OPT_ABLATION bit mask (bkr.h): 0 = the full method
+    int tune[BKR_TUNE_COUNT]; // BKR_OPT_TUNE + k (bkr.h): launch parameters, 0 = default
     SolverFlags *api_flags; // device flags for the API-level fused update
     int dslash_nblock;  // rhs count of the whole block while launch_dslash works through it in chunks (L2 blocking uses it)
     int dslash_variant; // last stencil kernel used: 0 plain, 1 window, -1 none yet

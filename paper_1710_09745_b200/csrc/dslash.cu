@@ -269,8 +269,7 @@ static int launch_tg(bkr_ctx *ctx, int parity, int N, const void *in, void *out,
     const int ntiles = link_tiles(ctx->g);
     const Cx *wt = (sizeof(Real) == 8 ? (const Cx *)ctx->links64 : (const Cx *)ctx->links32) +
                    (size_t)parity * ntiles * 16 * 9 * BKR_LINK_TILE;
-    static const char *oenv = getenv("BKR_DSLASH_OPTS");
-    const int opts = oenv ? atoi(oenv) : 0;
+    const int opts = 0;
     dim3 block(BKR_LINK_TILE, G);
     unsigned grid = (unsigned)std::min(ntiles, BKR_NUM_SMS * MINB);
     static int attr_dev = -1; // per instantiation: the opt-in is per device
@@ -296,23 +295,6 @@ template <typename Real>
 static int launch_n(bkr_ctx *ctx, int parity, int N, const void *in, void *out, const void *xp, double a, const int *done)
 {
 #define GO(T_, G_, M_) return launch_tg<Real, T_, G_, M_>(ctx, parity, N, in, out, xp, a, done)
-#ifdef BKR_TUNING
-    static const char *cfg = getenv("BKR_DSLASH_CFG"); // tuning hook (build with -DBKR_TUNING): "T,G,MINB,D,RG"
-    if (cfg) {
-        int t = 0, gg = 0, mb = 0, dd = 0, rg = 0;
-        sscanf(cfg, "%d,%d,%d,%d,%d", &t, &gg, &mb, &dd, &rg);
-        if (N <= t * gg) {
-#define TRY(T_, G_, M_, D_, R_) if (t == T_ && gg == G_ && mb == M_ && dd == D_ && rg == R_) return launch_tg<Real, T_, G_, M_, D_, R_>(ctx, parity, N, in, out, xp, a, done)
-            TRY(8, 2, 2, 12, 2); TRY(8, 2, 2, 12, 4); TRY(8, 2, 2, 12, 8); TRY(8, 2, 3, 6, 4); TRY(8, 2, 3, 6, 8); TRY(8, 2, 2, 8, 8);
-            TRY(4, 4, 2, 12, 8); TRY(4, 4, 2, 6, 8); TRY(4, 4, 1, 24, 16); TRY(4, 4, 2, 12, 4); TRY(4, 4, 1, 12, 16);
-            TRY(8, 1, 4, 12, 4); TRY(8, 1, 3, 12, 8); TRY(8, 1, 2, 12, 16); TRY(4, 2, 4, 12, 4); TRY(4, 2, 3, 12, 8); TRY(4, 2, 2, 24, 16);
-            TRY(8, 4, 1, 12, 16); TRY(8, 4, 1, 12, 8); TRY(4, 8, 1, 12, 16); TRY(4, 8, 1, 6, 16); TRY(8, 3, 1, 12, 16); TRY(4, 6, 1, 12, 16);
-#undef TRY
-            fprintf(stderr, "BKR_DSLASH_CFG %s: not compiled in\n", cfg);
-            return BKR_EINVAL;
-        }
-    }
-#endif
     // Register budget decides the shape (ptxas -v: the fp64 T = 8 thread needs ~190 registers for 48 accumulators, the
     // 12-deep load ring and the link column; under a 168-register cap it spills ~0.5 KB per thread, and ncu showed the
     // spill traffic, not the stencil, filling the LSU).  fp64: at most 2 CTAs of 128 threads (or 4 of 64) per SM.

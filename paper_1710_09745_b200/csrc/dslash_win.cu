@@ -3,28 +3,41 @@
 //   out(x) = sum_h W_h(x) in(nbr_h(x)),  16 hops;  optional epilogue out = a * xp - out
 //
 // Why a second kernel.  With every neighbour vector fetched from L2 by plain loads
-// (dslash.cu) each input element crosses the L2 -> SM fabric 16 times per call; at N >= 8 that is 8.6-14.4 GB per
-// launch at 32^3 x 64 and the kernel sits on the ~6300 B/clk L2-slice throughput cap of the chip, not on HBM (ncu:
-// lts__t_sectors ~ 3.8e8 per launch, DRAM 48 %, FP64 pipe 39 %).  The paper's answer on Pascal was texture/L1 reuse
-// between the rhs of a thread block; on B200 the per-hop footprint (N x 48 bytes per site) is too
-// large for L1 to hold between hops, so the reuse is made explicit:
+// (dslash.cu) each input element crosses the L2 -> SM fabric 16 times per call and the per-hop footprint (N x 48
+// bytes per site) is too large for L1 to hold between hops; the reuse the paper got from the texture cache
+// is made explicit:
 //  * A CTA walks a run of consecutive 64-site tiles inside one (z, t) "strip" (all x, y at fixed z, t).  The x- and
 //    y-neighbours of a tile lie within +-3 x-rows of it, so a sliding WINDOW of input rows in shared memory serves
 //    all 8 x/y hops: every input row is fetched from L2 once per strip instead of 8 times.  z/t hops still cost one
 //    L2 fetch each: 9 fetches per site instead of 16.
-//  * Nothing is loaded by the arithmetic warps.  One producer lane feeds three shared-memory rings with TMA:
-//    links (1-D bulk copy, 9 x 64 complex per hop, as in dslash.cu), window chunks (3-D tensor copy: 32 sites x 3
-//    colours x NC rhs) and z/t neighbour stages (tensor copy: 64 sites x 3 colours x NC rhs, shifted by the hop).
-//  * A CTA holds NC = T G rhs (8 in fp64, 16 in fp32).  For N > NC a thread-block CLUSTER of C = ceil(N / NC) CTAs
+//  * Apart from the xpay operand (3 T / 2 streaming loads per thread, issued at the start of a tile), nothing is loaded
+//    from global memory by the arithmetic warps.  Producer lanes (one per warp of two producer warpgroups, 48 registers
+//    each after setmaxnreg) feed two shared-memory rings with TMA.  The HOP-STAGE ring holds, per hop pair (h, 8 + h)
+//    of a tile, the links of both hops (1-D bulk copies, 9 x 64 complex each) and the z/t neighbour tile of hop 8 + h
+//    as two 32-site chunks (3-D tensor copies: 32 sites x 3 colours x NC rhs); the four parts have one lane each (a
+//    lane issues at most one bulk copy per ~360 cycles) and complete on ONE full barrier.  The WINDOW ring holds the
+//    32-site chunks of the strip.
+//  * A CTA holds NC = 2 T rhs (8 in fp64, 16 in fp32).  For N > NC a thread-block CLUSTER of C = ceil(N / NC) CTAs
 //    works on the same tiles, one rhs slice each, and every link stage is fetched ONCE for the cluster: each CTA
 //    issues 1/C of the stage as a multicast bulk copy into all C shared memories (the paper's "load each link once
 //    and reuse it across the rhs", across SMs).  Consumers release a link slot by arriving on the
 //    empty barrier of every CTA of the cluster.
-//  * The 16 hops are split between two warp sets with private accumulators: set A does the 8 x/y hops from the
-//    window, set B the 8 z/t hops from the sub-stage ring; B hands its partial sums to A through shared memory once
-//    per tile.  Two independent instruction streams per SM sub-partition hide each other's shared-memory latency.
+//  * The 16 hops are split inside every arithmetic warp: lanes 0-15 do the 8 x/y hops of 16 sites from the window,
+//    lanes 16-31 the 8 z/t hops of the same 16 sites from the stage ring -- one instruction stream, only the
+//    operand addresses differ -- and the two partial sums meet through 6 T warp shuffles per lane; each half then
+//    stores half of the rhs.  (Round 1 gave the two hop sets to different warps, which met through a 24 KB
+//    shared-memory buffer and a pair of barriers; the buffer and the barriers are gone.)
 //  * The window is cyclic in y (virtual chunk c of a strip = memory chunk c mod chunks-per-strip), so the wrapped
 //    y-neighbours of the first and last rows of a strip come from the window like all others.
+// What the box measured and this kernel is built around (profiles/r2_onchip_probes.md):
+//  * every LDS.128 return costs 4-5 cycles of the register-file write port of its scheduler, the same port the DFMA
+//    results use, broadcast or not; with operands from shared memory the FP64 pipe tops out at ~48 of 64 DFMA/clk/SM
+//    for T = 4, 6, 8 alike;
+//  * TMA fills do not compete with LDS for the shared-memory port (3 % loss), plain global loads do (1:1);
+//  * a TMA round trip is 500-700 cycles from L2 on an idle chip, 1300-2500 under load: ring depth decides whether the
+//    arithmetic warps wait;
+//  * cp.async.bulk.prefetch.L2 of the link stream one to three tiles ahead made the kernel 20-50 % SLOWER (tried
+//    twice, with and without the evict-first policy) and is not used.
 #include "common.cuh"
 #include "tma.cuh"
 
@@ -33,13 +46,14 @@
 #include <algorithm>
 #include <stdlib.h>
 #include <string.h>
+#include <type_traits>
 #include <vector>
 
 #define WIN_CHUNK 32 /* sites per window chunk */
-#ifndef WIN_HOP_UNROLL
-#define WIN_HOP_UNROLL 1
-#endif
-static constexpr int HOP_UNROLL = WIN_HOP_UNROLL; // hop loops of the arithmetic warps (2 and 8 measured: no gain)
+#define WIN_CONSUMER_WARPS 8
+#define WIN_PRODUCER_WARPS 8
+#define WIN_THREADS ((WIN_CONSUMER_WARPS + WIN_PRODUCER_WARPS) * 32)
+#define WIN_CONSUMER_REGS 208 /* 256 x 208 + 256 x 48 = 65536 */
 
 struct WinParams {
     Geom g;
@@ -53,12 +67,10 @@ struct WinParams {
     const int *done;
     int HcL;    // window reach below/above a tile, in chunks
     int WCH;    // window ring slots (chunks)
-    int nzlog;  // log2 of the z/t stage ring depth
-    int rllog;  // log2 of the link ring depth (2 or 3)
+    int D;      // hop-stage ring depth
     int xover;  // 1: tiles do not start on x-row boundaries (64 % (X/2) != 0): x hops read the chunk below the tile
     int slim;   // 1: window without spare slots (chunks below the tile released after the y-3, y-1 hops)
-    int opts;   // tuning bits (BKR_WIN_OPTS): 1 = L2 prefetch of the next tile's links, 2 = of its z/t stages (no gain measured)
-    uint32_t off_win, off_zt, off_red, off_bar;
+    uint32_t off_win, off_bar;
 };
 
 // ---------------------------------------------------------------- PTX helpers (cluster, tensor TMA)
@@ -97,85 +109,116 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *tm, in
                  "l"(tm), "r"(smem_addr(bar)), "r"(c0), "r"(c1), "r"(c2)
                  : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_1d(const void *src, uint32_t bytes)
+// blocking wait with a long suspend-time hint: the thread sleeps in hardware until the phase completes instead of
+// spinning (ncu: with the default hint the producer lanes executed a third of all instructions of the kernel and
+// took issue slots from the arithmetic warps of their schedulers)
+__device__ __forceinline__ void mbar_wait_slow(uint64_t *bar, uint32_t parity)
 {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"(
+                     smem_addr(bar)),
+                 "r"(parity), "r"(0x989680)
+                 : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *tm, int c0, int c1, int c2)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(tm), "r"(c0), "r"(c1), "r"(c2) : "memory");
-}
-__device__ __forceinline__ void mbar_wait_mem(uint64_t *bar, uint32_t parity)
+// one non-blocking probe of a barrier phase (test_wait); the result is consumed later (mbar_finish) so that FMAs can
+// issue in between
+__device__ __forceinline__ uint32_t mbar_try(uint64_t *bar, uint32_t parity)
 {
     uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(smem_addr(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok)
+                 : "r"(smem_addr(bar)), "r"(parity));
+    return ok;
 }
-__device__ __forceinline__ void mbar_arrive_mem(uint64_t *bar)
+__device__ __forceinline__ void mbar_finish(uint32_t ok, uint64_t *bar, uint32_t parity)
 {
-    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+    if (!ok)
+        asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"(
+                         smem_addr(bar)),
+                     "r"(parity), "r"(0x989680));
+}
+// streaming 16 / 8-byte global load of the xpay operand (read once per call)
+__device__ __forceinline__ double2 ldg_stream(const double2 *p)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float2 ldg_stream(const float2 *p)
+{
+    float2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+    return v;
 }
 
-// acc_a += W_ab v_b for one rhs: u[a] = W_ab (a = 0..2), v = in_b
-template <typename Real, typename Cx> __device__ __forceinline__ void cfma3(Real (&acc)[6], const Cx (&u)[3], const Cx v)
+// acc[i] += W(:, b) v_i(b) for the T rhs of a thread: u[a] = W_ab, v[i] = component b of rhs i
+template <typename Real, typename Cx, int T> __device__ __forceinline__ void col_fma(Real (&acc)[T][6], const Cx (&u)[3], const Cx (&v)[T])
 {
 #pragma unroll
-    for (int aa = 0; aa < 3; aa++) {
-        acc[2 * aa] = fma(u[aa].x, v.x, acc[2 * aa]);
-        acc[2 * aa + 1] = fma(u[aa].x, v.y, acc[2 * aa + 1]);
-    }
+    for (int i = 0; i < T; i++)
 #pragma unroll
-    for (int aa = 0; aa < 3; aa++) {
-        acc[2 * aa] = fma(-u[aa].y, v.y, acc[2 * aa]);
-        acc[2 * aa + 1] = fma(u[aa].y, v.x, acc[2 * aa + 1]);
-    }
+        for (int a = 0; a < 3; a++) {
+            acc[i][2 * a] = fma(u[a].x, v[i].x, acc[i][2 * a]);
+            acc[i][2 * a + 1] = fma(u[a].x, v[i].y, acc[i][2 * a + 1]);
+        }
+#pragma unroll
+    for (int i = 0; i < T; i++)
+#pragma unroll
+        for (int a = 0; a < 3; a++) {
+            acc[i][2 * a] = fma(-u[a].y, v[i].y, acc[i][2 * a]);
+            acc[i][2 * a + 1] = fma(u[a].y, v[i].x, acc[i][2 * a + 1]);
+        }
 }
+// 16 / 8-byte shared-memory load at a shared-space address plus an immediate offset
+template <typename Cx> __device__ __forceinline__ Cx lds_at(uint32_t addr, uint32_t off);
+template <> __device__ __forceinline__ double2 lds_at<double2>(uint32_t addr, uint32_t off)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr + off));
+    return v;
+}
+template <> __device__ __forceinline__ float2 lds_at<float2>(uint32_t addr, uint32_t off)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr + off));
+    return v;
+}
+__device__ __forceinline__ double shfl_x16(double v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
+__device__ __forceinline__ float shfl_x16(float v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
 
-// blockDim = (4 G + 4) warps: warps [0, 2G) = set A (x/y hops), [2G, 4G) = set B (z/t hops), last 4 warps = producers.
-// Inside a set, warp w handles sites (w % 4) * 16 + lane % 16 of the 64-site tile and the rhs groups 2 (w / 4) + lane / 16
-// (T rhs each); for odd G: rhs group w / 2 and sites (w % 2) * 32 + lane.
-template <typename Real, int T, int G, int C, bool XP>
-__global__ void __launch_bounds__((4 * G + 4) * 32, 1)
-dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_constant__ CUtensorMap tm_zt,
-                  const __grid_constant__ CUtensorMap tm_xp, const WinParams p)
+// blockDim = 16 warps: warps 0-7 arithmetic, warps 8-15 producers (lane 0 of warps 8-13 works).
+// Arithmetic warp w: sites (w % 4) * 16 + lane % 16 of the 64-site tile, rhs group w / 4 (T rhs), hop set lane / 16.
+// A HOP STAGE of the ring holds everything hop pair (h, 8 + h) of a tile needs besides the window:
+//   [ links of hop h : 9 x 64 | links of hop 8 + h : 9 x 64 | z/t neighbours of hop 8 + h: 2 chunks of NC x 3 x 32 ]
+// filled by four producer lanes (one bulk / tensor copy each) that signal ONE full barrier, released by ONE arrival
+// per arithmetic warp (per CTA of the cluster: the link parts are multicast).
+template <typename Real, int T, int C, bool XP>
+__global__ void __launch_bounds__(WIN_THREADS, 1)
+dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
 {
     typedef typename CxT<Real>::type Cx;
-    constexpr int NC = T * G;
-    constexpr int NWS = 2 * G;
+    constexpr int NC = 2 * T;
+    constexpr int NW = WIN_CONSUMER_WARPS;
     constexpr uint32_t LSTAGE = 9 * 64 * sizeof(Cx);
     constexpr uint32_t WCHUNK = NC * 3 * WIN_CHUNK * sizeof(Cx);
-    constexpr uint32_t ZSTAGE = NC * 3 * 64 * sizeof(Cx); // one z/t hop: [rhs][colour][64 sites]
+    constexpr uint32_t HSTAGE = 2 * LSTAGE + 2 * WCHUNK;
+    constexpr uint32_t PLANE = WIN_CHUNK * sizeof(Cx); // bytes between the (rhs, colour) planes of a chunk
     extern __shared__ __align__(1024) unsigned char dsm[];
-    unsigned char *const lnk = dsm;
+    unsigned char *const stg = dsm;
     unsigned char *const win = dsm + p.off_win;
-    unsigned char *const zt = dsm + p.off_zt;
-    Cx *const red = reinterpret_cast<Cx *>(dsm + p.off_red); // [NC * 3][64]
     uint64_t *const bar = reinterpret_cast<uint64_t *>(dsm + p.off_bar);
-    uint64_t *const lfull = bar, *const lempty = bar + 8, *const wfull = bar + 16, *const wempty = bar + 32,
-                    *const zfull = bar + 48, *const zempty = bar + 56, *const redfull = bar + 64, *const redempty = bar + 65;
+    uint64_t *const hfull = bar, *const hempty = bar + 8, *const wfull = bar + 16, *const wempty = bar + 32;
     if (p.done && *p.done) return;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int nzlog = p.nzlog, NZ = 1 << nzlog, rllog = p.rllog, RL = 1 << rllog, WCH = p.WCH, HcL = p.HcL;
+    const int D = p.D, WCH = p.WCH, HcL = p.HcL;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < RL; s++) {
-            mbar_init(&lfull[s], 1);
-            mbar_init(&lempty[s], NWS * C);
+        for (int s = 0; s < D; s++) {
+            mbar_init(&hfull[s], 4);
+            mbar_init(&hempty[s], NW * C);
         }
         for (int s = 0; s < WCH; s++) {
             mbar_init(&wfull[s], 1);
-            mbar_init(&wempty[s], NWS);
+            mbar_init(&wempty[s], NW);
         }
-        for (int s = 0; s < NZ; s++) {
-            mbar_init(&zfull[s], 1);
-            mbar_init(&zempty[s], NWS);
-        }
-        mbar_init(redfull, NWS * 32);
-        mbar_init(redempty, NWS * 32);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (C > 1) cluster_sync_all();
@@ -186,285 +229,290 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const __grid_const
     const Geom &g = p.g;
     const int Xh = g.X[0] >> 1;
     const int Vh = g.Vh;
+    const int XhY = Xh * g.X[1];
 
-    constexpr int npt = XP ? 9 : 8; // z/t ring stages per tile: 8 hops + the xp tile of the epilogue
-    const bool dry = (p.opts & 4) != 0; // tuning probe: no producers, no barriers (results are garbage)
-    if (warp >= 2 * NWS) {
-        // ------------------------------------------------------------------ producers: one lane in each of 4 warps
-        //   role 0: link stages of set A (even sequence numbers)
-        //   role 1: link stages of set B (odd sequence numbers)
-        //   role 2: z/t neighbour stages (and the xp tile of the epilogue)
-        //   role 3: window chunks
-        // Each ring has its own in-order issuer, so a full ring never blocks the refill of another one.  Every
-        // stage is also requested into L2 one tile ahead (cp.async.bulk.prefetch.L2): the HBM latency is paid there,
-        // the shared-memory rings only have to cover the L2 -> SM latency.
-        const int role = warp - 2 * NWS;
-        if (lane == 0 && !dry) {
+    if (warp >= NW) {
+        // ------------------------------------------------------------------ producers: lane 0 of five warps
+        //   role 0: links of the x/y hops        role 1: links of the z/t hops
+        //   role 2, 3: lower / upper 32-site chunk of the z/t neighbour tile
+        //   role 4: window chunks
+        // (one lane issues at most one bulk copy per ~360 cycles, measured: hence one lane per part of a stage)
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 48;");
+        const int role = warp - NW;
+        if (lane == 0 && role < 5) {
             const uint64_t pol = policy_evict_first();
             const Cx *wt = reinterpret_cast<const Cx *>(p.wt);
-            const int XhY = Xh * g.X[1];
             constexpr uint32_t SL = LSTAGE / C; // this CTA's slice of a link stage
-            // neighbour tile start (even-odd index) of tile k for z/t hop h
-            auto zt_src = [&](int k, int h) {
-                const int e0 = k * 64;
-                const int zc = (e0 / XhY) % g.X[2], tcd = e0 / (XhY * g.X[2]);
-                const int mu = BKR_HOP_MU(h), hop = BKR_HOP_LONG(h) ? 3 : 1;
-                const int cm = mu == 2 ? zc : tcd, Xm = mu == 2 ? g.X[2] : g.X[3];
-                const int smh = mu == 2 ? XhY : XhY * g.X[2];
-                int cn = BKR_HOP_BACK(h) ? cm - hop : cm + hop;
-                if (cn < 0) cn += Xm;
-                if (cn >= Xm) cn -= Xm;
-                return e0 + (cn - cm) * smh;
-            };
-            int tc = 0, wslot = 0, wuse = 0;
+            int wslot = 0, wuse = 0;
+            int hslot = 0, huse = 0; // hop-stage ring position (roles 0-3)
             for (int si = cid; si < p.nseg; si += ncl) {
                 const int4 sg = p.segs[si];
                 const int seg_lo = 2 * sg.x - HcL, seg_hi = 2 * sg.y - 1 + HcL; // virtual (cyclic in y) chunks
                 const int cs = 2 * sg.z, ncs = 2 * (sg.w - sg.z + 1);
-                auto chunk_site0 = [&](int c, int cs_, int ncs_) { // memory site of virtual chunk c of a strip
-                    int r = (c - cs_) % ncs_;
-                    if (r < 0) r += ncs_;
-                    return (cs_ + r) * WIN_CHUNK;
-                };
-                const bool has_next = si + ncl < p.nseg;
-                int4 sn = sg;
-                if (has_next) sn = p.segs[si + ncl];
                 int next_c = seg_lo;
-                for (int k = sg.x; k < sg.y; k++, tc++) {
-                    const int knext = k + 1 < sg.y ? k + 1 : (has_next ? sn.x : -1); // this CTA's next tile
-                    if (role == 2) {
-                        for (int j = 0; j < npt; j++) {
-                            const int zs = npt * tc + j, slot = zs & (NZ - 1), use = zs >> nzlog;
-                            if (use > 0) mbar_wait(&zempty[slot], (use - 1) & 1);
-                            mbar_expect_tx(&zfull[slot], ZSTAGE);
-                            if (j < 8) tma_load_3d(zt + (size_t)slot * ZSTAGE, &tm_zt, 2 * zt_src(k, 8 + j), 0, (int)rank * NC, &zfull[slot]);
-                            else tma_load_3d(zt + (size_t)slot * ZSTAGE, &tm_xp, 2 * k * 64, 0, (int)rank * NC, &zfull[slot]);
-                            if (j < 8 && knext >= 0 && (p.opts & 2)) tma_prefetch_3d(&tm_zt, 2 * zt_src(knext, 8 + j), 0, (int)rank * NC);
-                        }
-                        continue;
-                    }
-                    if (role == 3) {
+                // z/t neighbour offsets (in sites) of the strip, hop j = 0..7: z-3, z-1, z+1, z+3, t-3, t-1, t+1, t+3
+                const int zc = (sg.z * 64 / XhY) % g.X[2], tcd = sg.z * 64 / (XhY * g.X[2]);
+                for (int k = sg.x; k < sg.y; k++) {
+                    if (role == 4) {
                         // window chunks, up to what the NEXT tile needs, as far ahead as free slots allow
                         const int hi = min(2 * k + 3 + HcL, seg_hi);
                         while (next_c <= hi) {
-                            if (wuse > 0) mbar_wait(&wempty[wslot], (wuse - 1) & 1);
+                            int r = (next_c - cs) % ncs; // memory chunk of virtual chunk next_c of the strip
+                            if (r < 0) r += ncs;
+                            if (wuse > 0) mbar_wait_slow(&wempty[wslot], (wuse - 1) & 1);
                             mbar_expect_tx(&wfull[wslot], WCHUNK);
-                            tma_load_3d(win + (size_t)wslot * WCHUNK, &tm_win, 2 * chunk_site0(next_c, cs, ncs), 0, (int)rank * NC, &wfull[wslot]);
+                            tma_load_3d(win + (size_t)wslot * WCHUNK, &tm_win, 2 * (cs + r) * WIN_CHUNK, 0, (int)rank * NC, &wfull[wslot]);
                             next_c++;
                             if (++wslot == WCH) {
                                 wslot = 0;
                                 wuse++;
                             }
                         }
-                        if (k == sg.y - 1 && has_next) // first window of the next segment -> L2
-                            for (int cc = 2 * sn.x - HcL; cc <= 2 * sn.x + 1 + HcL; cc++)
-                                tma_prefetch_3d(&tm_win, 2 * chunk_site0(cc, 2 * sn.z, 2 * (sn.w - sn.z + 1)), 0, (int)rank * NC);
                         continue;
                     }
                     for (int j = 0; j < 8; j++) {
-                        const int h = role ? 8 + j : j;
-                        const int ls = 16 * tc + 2 * j + role, slot = ls & (RL - 1), use = ls >> rllog;
-                        if (use > 0) mbar_wait(&lempty[slot], (use - 1) & 1);
-                        mbar_expect_tx(&lfull[slot], LSTAGE);
-                        const unsigned char *src = reinterpret_cast<const unsigned char *>(wt + ((size_t)k * 16 + h) * 9 * 64);
-                        if (C == 1)
-                            tma_load_1d_hint(lnk + (size_t)slot * LSTAGE, src, LSTAGE, &lfull[slot], pol);
-                        else
-                            tma_load_1d_mc(lnk + (size_t)slot * LSTAGE + rank * SL, src + rank * SL, SL, &lfull[slot],
-                                           (uint16_t)((1u << C) - 1u), pol);
-                        if (knext >= 0 && (p.opts & 1))
-                            tma_prefetch_1d(reinterpret_cast<const unsigned char *>(wt + ((size_t)knext * 16 + h) * 9 * 64) + rank * SL, SL);
+                        if (huse > 0) mbar_wait_slow(&hempty[hslot], (huse - 1) & 1);
+                        unsigned char *const sb = stg + (size_t)hslot * HSTAGE;
+                        if (role < 2) {
+                            const int h = role ? 8 + j : j;
+                            unsigned char *const dst = sb + role * LSTAGE;
+                            mbar_expect_tx(&hfull[hslot], LSTAGE);
+                            const unsigned char *src = reinterpret_cast<const unsigned char *>(wt + ((size_t)k * 16 + h) * 9 * 64);
+                            if (C == 1) tma_load_1d_hint(dst, src, LSTAGE, &hfull[hslot], pol);
+                            else tma_load_1d_mc(dst + rank * SL, src + rank * SL, SL, &hfull[hslot], (uint16_t)((1u << C) - 1u), pol);
+                        } else {
+                            const bool isz = j < 4;
+                            const int hop = 2 * (j & 3) - 3;
+                            const int cm = isz ? zc : tcd, Xm = isz ? g.X[2] : g.X[3];
+                            int cn = cm + hop;
+                            if (cn < 0) cn += Xm;
+                            if (cn >= Xm) cn -= Xm;
+                            const int e0 = k * 64 + (cn - cm) * (isz ? XhY : XhY * g.X[2]) + (role - 2) * WIN_CHUNK;
+                            mbar_expect_tx(&hfull[hslot], WCHUNK);
+                            tma_load_3d(sb + 2 * LSTAGE + (role - 2) * WCHUNK, &tm_win, 2 * e0, 0, (int)rank * NC, &hfull[hslot]);
+                        }
+                        if (++hslot == D) {
+                            hslot = 0;
+                            huse++;
+                        }
                     }
                 }
             }
         }
-    } else if (warp < NWS) {
-        // ------------------------------------------------------------------ set A: x/y hops from the window
-        // The window is cyclic in y: virtual chunk c of a strip is memory chunk cs + (c - cs) mod ncs, so the wrapped
-        // neighbours of the first and last rows of a strip are served like all others (no global loads here at all).
-        // lanes 0-15 and 16-31 of a warp: the same 16 sites, two rhs groups -- the link loads of the two half-warps hit the
-        // same shared-memory addresses (one broadcast wavefront pair instead of two): half the link traffic on the port
-        const int sl = (G % 2 == 0) ? (warp & 3) * 16 + (lane & 15) : (warp & 1) * 32 + lane;
-        const int j0 = (G % 2 == 0) ? (2 * (warp >> 2) + (lane >> 4)) * T : (warp >> 1) * T;
-        int tc = 0, q0 = 0;
+    } else {
+        // ------------------------------------------------------------------ arithmetic warps
+        // Software pipeline: the operands of a COLUMN (3 link elements W_ab, a = 0..2, and the T vector elements of
+        // colour b) are loaded one column ahead of the 12 T FMAs that use them, into the register set (A or B) the
+        // running column does not use; the barrier probe is issued a column ahead as well.  Two hops = six columns bring
+        // the register roles back to where they started, so nothing is ever copied; the hop index is a compile-time
+        // constant (a runtime hop loop cost 280 non-FMA instructions per hop and warp, ncu).
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WIN_CONSUMER_REGS));
+        const int set = lane >> 4;                     // 0: x/y hops from the window, 1: z/t hops from the stage ring
+        const int sl = (warp & 3) * 16 + (lane & 15);  // site in tile
+        const int j0 = (warp >> 2) * T;                // first rhs of this thread inside the CTA's slice
+        const int jg = (int)rank * NC + j0;
+        const int io = set ? T / 2 : 0;                // first rhs (inside the thread's T) this lane stores
+        // this lane's link column base inside a hop stage, and (set 1) its z/t operand
+        const uint32_t lkoff = (uint32_t)set * LSTAGE + (uint32_t)sl * (uint32_t)sizeof(Cx);
+        const uint32_t ztoff = 2 * LSTAGE + (uint32_t)(sl >> 5) * WCHUNK + (uint32_t)(j0 * 3 * WIN_CHUNK + (sl & 31)) * (uint32_t)sizeof(Cx);
+        const uint32_t woff = (uint32_t)(j0 * 3 * WIN_CHUNK) * (uint32_t)sizeof(Cx);
+        Cx uA[3], uB[3], vA[T], vB[T];
+        // operand addresses are 32-bit shared-space integers: one base register per hop, immediate offsets per load
+        auto load_u = [&](Cx(&u)[3], uint32_t lk, int b) {
+#pragma unroll
+            for (int aa = 0; aa < 3; aa++) u[aa] = lds_at<Cx>(lk, (uint32_t)((3 * aa + b) * 64) * (uint32_t)sizeof(Cx));
+        };
+        auto load_v = [&](Cx(&v)[T], uint32_t vp, int b) {
+#pragma unroll
+            for (int i = 0; i < T; i++) v[i] = lds_at<Cx>(vp, (uint32_t)(i * 3 + b) * PLANE);
+        };
+        const uint32_t stg_s = smem_addr(stg), win_s = smem_addr(win);
+        int hslot = 0; // hop-stage ring position
+        uint32_t hph = 0;
+        auto release_stage = [&](int s_) {
+            __syncwarp();
+            if (C == 1) {
+                if (lane == 0) mbar_arrive(&hempty[s_]);
+            } else {
+                if (lane < C) mbar_arrive_remote(&hempty[s_], (uint32_t)lane);
+            }
+        };
+        auto advance = [&]() {
+            if (++hslot == D) {
+                hslot = 0;
+                hph ^= 1u;
+            }
+        };
+        // Window bookkeeping without divisions: ring positions (slot, phase) of the next chunk to wait for, of the next
+        // chunk to release and of the first chunk of the current tile advance by conditional subtraction; the position of
+        // the site in its x-row (ex, row parity) is divided out once per segment and stepped per tile.
+        int wq_slot = 0;     // ring slot of the next chunk to wait for
+        uint32_t wq_ph = 0;  // its phase
+        int rl_slot = 0;     // ring slot of the next chunk to release
+        const int dex = 64 % Xh, drow = 64 / Xh; // a tile further: ex += dex (mod Xh), row += drow (+ carry)
         for (int si = cid; si < p.nseg; si += ncl) {
             const int4 sg = p.segs[si];
             const int seg_lo = 2 * sg.x - HcL, seg_hi = 2 * sg.y - 1 + HcL; // virtual chunks of this segment
-            const int strip_sites = (sg.w - sg.z + 1) * 64;
+            const int zpar = ((sg.z * 64 / XhY) % g.X[2] + sg.z * 64 / (XhY * g.X[2]) + p.parity) & 1; // (z + t + parity) of the strip
             int waited = seg_lo, released = seg_lo;
-            for (int k = sg.x; k < sg.y; k++, tc++) {
+            // slot of the first chunk of tile sg.x: HcL chunks behind the segment's first chunk (= the next to wait for)
+            int t_slot = wq_slot + HcL;
+            if (t_slot >= WCH) t_slot -= WCH;
+            int ex, rowp;
+            {
+                const int el = sg.x * 64 + sl - sg.z * 64; // site inside the strip
+                ex = el % Xh;
+                rowp = (el / Xh + zpar) & 1;
+            }
+            auto release_to = [&](int new_rel) { // lane 0: give the chunks [released, new_rel) back to the window producer
+                for (; released < new_rel; released++) {
+                    mbar_arrive(&wempty[rl_slot]);
+                    if (++rl_slot == WCH) rl_slot = 0;
+                }
+            };
+            for (int k = sg.x; k < sg.y; k++) {
+                const int e = k * 64 + sl;
+                // xpay operand of the rhs this lane will store: requested now, used after the 16 hops
+                Cx xv[XP ? T / 2 : 1][3];
+                if (XP) {
+                    const Cx *xsrc = reinterpret_cast<const Cx *>(p.xp) + (size_t)min(jg + io, p.N - 1) * 3 * Vh + e;
+#pragma unroll
+                    for (int i = 0; i < T / 2; i++)
+#pragma unroll
+                        for (int cc = 0; cc < 3; cc++) xv[i][cc] = ldg_stream(xsrc + (size_t)((jg + io + i < p.N ? i : 0) * 3 + cc) * Vh);
+                }
                 const int whi = 2 * k + 1 + HcL;
                 while (waited <= whi) {
-                    const int qq = q0 + waited - seg_lo;
-                    if (!dry) mbar_wait(&wfull[qq % WCH], (qq / WCH) & 1);
+                    mbar_wait(&wfull[wq_slot], wq_ph);
+                    if (++wq_slot == WCH) {
+                        wq_slot = 0;
+                        wq_ph ^= 1u;
+                    }
                     waited++;
                 }
-                const int slot2k = (q0 + 2 * k - seg_lo) % WCH;
-                const int e = k * 64 + sl;
-                int s = 2 * e;
-                int c0, c1;
-                {
-                    const int x0 = s % g.X[0];
-                    int r = s / g.X[0];
-                    c1 = r % g.X[1];
-                    r /= g.X[1];
-                    const int c2 = r % g.X[2], c3 = r / g.X[2];
-                    c0 = x0 + ((c1 + c2 + c3 + p.parity) & 1);
-                    s = s - x0 + c0;
-                }
+                const int slot2k = t_slot;
+                const int par = rowp; // x = 2 ex + par
+                // vector operand of hop h (h < 8) of this lane's set: window address (set 0) or stage offset (set 1)
+                auto win_ptr = [&](int h) -> uint32_t {
+                    const int mu = BKR_HOP_MU(h), hop = BKR_HOP_LONG(h) ? 3 : 1, sgn = BKR_HOP_BACK(h) ? -hop : hop;
+                    int d;
+                    if (mu == 1) {
+                        d = sl + sgn * Xh;
+                    } else {
+                        int cx = ex + ((par + sgn) >> 1); // column of the neighbour, periodic in x
+                        if (cx < 0) cx += Xh;
+                        if (cx >= Xh) cx -= Xh;
+                        d = sl + cx - ex;
+                    }
+                    int sidx = slot2k + (d >> 5); // arithmetic shift = floor
+                    if (sidx < 0) sidx += WCH;
+                    if (sidx >= WCH) sidx -= WCH;
+                    return win_s + (uint32_t)sidx * WCHUNK + woff + (uint32_t)(d & 31) * (uint32_t)sizeof(Cx);
+                };
                 Real acc[T][6];
 #pragma unroll
                 for (int i = 0; i < T; i++)
 #pragma unroll
                     for (int qd = 0; qd < 6; qd++) acc[i][qd] = (Real)0;
-#pragma unroll HOP_UNROLL
-                for (int h = 0; h < 8; h++) {
-                    const int mu = BKR_HOP_MU(h), hop = BKR_HOP_LONG(h) ? 3 : 1;
-                    const int cm = mu == 0 ? c0 : c1, Xm = mu == 0 ? g.X[0] : g.X[1], smh = mu == 0 ? 1 : g.X[0];
-                    int cn = BKR_HOP_BACK(h) ? cm - hop : cm + hop;
-                    if (cn < 0) cn += Xm;
-                    if (cn >= Xm) cn -= Xm;
-                    // neighbour position relative to the tile start, moved to its cyclic image inside the window
-                    int d = ((s + (cn - cm) * smh) >> 1) - k * 64;
-                    if (d >= 64 + WIN_CHUNK * HcL) d -= strip_sites;
-                    if (d < -WIN_CHUNK * HcL) d += strip_sites;
-                    int sidx = slot2k + (d >> 5); // arithmetic shift = floor
-                    if (sidx < 0) sidx += WCH;
-                    if (sidx >= WCH) sidx -= WCH;
-                    const Cx *wp = reinterpret_cast<const Cx *>(win + (size_t)sidx * WCHUNK) + j0 * 3 * WIN_CHUNK + (d & 31);
-                    const int ls = 16 * tc + 2 * h, slot = ls & (RL - 1);
-                    const Cx(*lk)[64] = reinterpret_cast<const Cx(*)[64]>(lnk + (size_t)slot * LSTAGE);
-                    if (!dry) mbar_wait(&lfull[slot], (ls >> rllog) & 1);
-                    // the whole 3 x 3 matrix goes to registers and the slot back to the producer before the arithmetic:
-                    // the ring then holds (almost) only data in flight
-                    Cx u[3][3]; // u[b][a] = W_ab
-#pragma unroll
-                    for (int b = 0; b < 3; b++)
-#pragma unroll
-                        for (int aa = 0; aa < 3; aa++) u[b][aa] = lds_cx(&lk[aa * 3 + b][sl]);
-                    __syncwarp();
-                    if (lane == 0 && !dry) {
-                        if (C == 1) mbar_arrive(&lempty[slot]);
-                        else
-                            for (uint32_t r = 0; r < (uint32_t)C; r++) mbar_arrive_remote(&lempty[slot], r);
-                    }
-#pragma unroll
-                    for (int b = 0; b < 3; b++) {
-                        Cx v[T];
-#pragma unroll
-                        for (int i = 0; i < T; i++) v[i] = lds_cx(wp + (i * 3 + b) * WIN_CHUNK);
-#pragma unroll
-                        for (int i = 0; i < T; i++) cfma3<Real, Cx>(acc[i], u[b], v[i]);
-                    }
-                    if (h == 1 && p.slim) {
+                mbar_wait(&hfull[hslot], hph);
+                uint32_t sb = stg_s + (uint32_t)hslot * HSTAGE;
+                uint32_t lk = sb + lkoff, vp = set ? sb + ztoff : win_ptr(0);
+                load_u(uA, lk, 0);
+                load_v(vA, vp, 0);
+                auto hop_pair = [&](auto HC) {
+                    constexpr int h = decltype(HC)::value;
+                    // ---- hop h (column 0 is in register set A)
+                    load_u(uB, lk, 1);
+                    load_v(vB, vp, 1);
+                    col_fma<Real, Cx, T>(acc, uA, vA);
+                    load_u(uA, lk, 2);
+                    load_v(vA, vp, 2);
+                    release_stage(hslot);
+                    advance();
+                    const uint32_t ok1 = mbar_try(&hfull[hslot], hph);
+                    const uint32_t sb1 = stg_s + (uint32_t)hslot * HSTAGE;
+                    const uint32_t vp1 = set ? sb1 + ztoff : win_ptr(h + 1);
+                    col_fma<Real, Cx, T>(acc, uB, vB);
+                    mbar_finish(ok1, &hfull[hslot], hph);
+                    const uint32_t lk1 = sb1 + lkoff;
+                    load_u(uB, lk1, 0);
+                    load_v(vB, vp1, 0);
+                    col_fma<Real, Cx, T>(acc, uA, vA);
+                    // ---- hop h + 1 (column 0 is in register set B)
+                    load_u(uA, lk1, 1);
+                    load_v(vA, vp1, 1);
+                    col_fma<Real, Cx, T>(acc, uB, vB);
+                    load_u(uB, lk1, 2);
+                    load_v(vB, vp1, 2);
+                    release_stage(hslot);
+                    if (h == 0 && p.slim) {
                         // hops 0, 1 are y-3, y-1 (common.cuh): the chunks below the tile are dead from here on and go back
                         // to the window producer, which loads the next tile's upper chunks into them
                         const int new_rel = 2 * k - p.xover; // x neighbours reach 2 sites below a tile that starts mid-row
-                        __syncwarp();
-                        if (lane == 0 && !dry)
-                            for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(q0 + cc - seg_lo) % WCH]);
-                        released = max(released, new_rel);
+                        // (after the __syncwarp of release_stage: every lane has issued its last read; every lane keeps the counters)
+                        if (lane == 0) release_to(new_rel);
+                        else
+                            for (; released < new_rel; released++)
+                                if (++rl_slot == WCH) rl_slot = 0;
                     }
-                }
+                    advance();
+                    if constexpr (h < 6) {
+                        const uint32_t ok2 = mbar_try(&hfull[hslot], hph);
+                        sb = stg_s + (uint32_t)hslot * HSTAGE;
+                        vp = set ? sb + ztoff : win_ptr(h + 2);
+                        col_fma<Real, Cx, T>(acc, uA, vA);
+                        mbar_finish(ok2, &hfull[hslot], hph);
+                        lk = sb + lkoff;
+                        load_u(uA, lk, 0);
+                        load_v(vA, vp, 0);
+                    } else {
+                        col_fma<Real, Cx, T>(acc, uA, vA);
+                    }
+                    col_fma<Real, Cx, T>(acc, uB, vB);
+                };
+                hop_pair(std::integral_constant<int, 0>{});
+                hop_pair(std::integral_constant<int, 2>{});
+                hop_pair(std::integral_constant<int, 4>{});
+                hop_pair(std::integral_constant<int, 6>{});
                 // release the window chunks the next tile of this segment does not need
                 {
                     const int new_rel = (k == sg.y - 1) ? seg_hi + 1 : 2 * (k + 1) - HcL;
                     __syncwarp();
-                    if (lane == 0 && !dry)
-                        for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(q0 + cc - seg_lo) % WCH]);
-                    released = max(released, new_rel);
+                    if (lane == 0) release_to(new_rel);
+                    else
+                        for (; released < new_rel; released++)
+                            if (++rl_slot == WCH) rl_slot = 0;
                 }
-                // hand the partial sums to set B, which finishes the tile
-                if (tc > 0 && !dry) mbar_wait_mem(redempty, (tc - 1) & 1);
+                // next tile of the segment: two chunks and 64 sites further
+                t_slot += 2;
+                if (t_slot >= WCH) t_slot -= WCH;
+                ex += dex;
+                rowp ^= drow & 1;
+                if (ex >= Xh) {
+                    ex -= Xh;
+                    rowp ^= 1;
+                }
+                // The two halves of the warp hold the x/y and the z/t part of the same (site, rhs) sums: each half sends the
+                // other the partial sums of the T / 2 rhs the other will store and adds what it receives to its own.
+                Cx *vout = reinterpret_cast<Cx *>(p.out) + (size_t)(jg + io) * 3 * Vh + e;
 #pragma unroll
-                for (int i = 0; i < T; i++)
+                for (int i = 0; i < T / 2; i++) {
 #pragma unroll
                     for (int cc = 0; cc < 3; cc++) {
+                        const Real sx = set ? acc[i][2 * cc] : acc[T / 2 + i][2 * cc];
+                        const Real sy = set ? acc[i][2 * cc + 1] : acc[T / 2 + i][2 * cc + 1];
+                        const Real mx = set ? acc[T / 2 + i][2 * cc] : acc[i][2 * cc];
+                        const Real my = set ? acc[T / 2 + i][2 * cc + 1] : acc[i][2 * cc + 1];
                         Cx o;
-                        o.x = acc[i][2 * cc];
-                        o.y = acc[i][2 * cc + 1];
-                        red[((j0 + i) * 3 + cc) * 64 + sl] = o;
-                    }
-                if (!dry) mbar_arrive_mem(redfull);
-            }
-            q0 += seg_hi - seg_lo + 1;
-        }
-    } else {
-        // ------------------------------------------------------------------ set B: z/t hops from the sub-stage ring,
-        // then the epilogue: add set A's partial sums, out = acc  or  a * xp - acc
-        const int wb = warp - NWS;
-        const int sl = (G % 2 == 0) ? (wb & 3) * 16 + (lane & 15) : (wb & 1) * 32 + lane;
-        const int j0 = (G % 2 == 0) ? (2 * (wb >> 2) + (lane >> 4)) * T : (wb >> 1) * T;
-        const int jg = (int)rank * NC + j0; // first global rhs of this thread
-        int tc = 0;
-        for (int si = cid; si < p.nseg; si += ncl) {
-            const int4 sg = p.segs[si];
-            for (int k = sg.x; k < sg.y; k++, tc++) {
-                const int e = k * 64 + sl;
-                Cx *vout = reinterpret_cast<Cx *>(p.out) + (size_t)jg * 3 * Vh + e;
-                Real acc[T][6];
-#pragma unroll
-                for (int i = 0; i < T; i++)
-#pragma unroll
-                    for (int qd = 0; qd < 6; qd++) acc[i][qd] = (Real)0;
-#pragma unroll HOP_UNROLL
-                for (int j = 0; j < 8; j++) {
-                    const int ls = 16 * tc + 2 * j + 1, slot = ls & (RL - 1);
-                    const Cx(*lk)[64] = reinterpret_cast<const Cx(*)[64]>(lnk + (size_t)slot * LSTAGE);
-                    if (!dry) mbar_wait(&lfull[slot], (ls >> rllog) & 1);
-                    Cx u[3][3];
-#pragma unroll
-                    for (int b = 0; b < 3; b++)
-#pragma unroll
-                        for (int aa = 0; aa < 3; aa++) u[b][aa] = lds_cx(&lk[aa * 3 + b][sl]);
-                    __syncwarp();
-                    if (lane == 0 && !dry) {
-                        if (C == 1) mbar_arrive(&lempty[slot]);
-                        else
-                            for (uint32_t r = 0; r < (uint32_t)C; r++) mbar_arrive_remote(&lempty[slot], r);
-                    }
-                    const int zs = npt * tc + j, zslot = zs & (NZ - 1);
-                    const Cx *zp = reinterpret_cast<const Cx *>(zt + (size_t)zslot * ZSTAGE) + j0 * 3 * 64 + sl;
-                    if (!dry) mbar_wait(&zfull[zslot], (zs >> nzlog) & 1);
-#pragma unroll
-                    for (int b = 0; b < 3; b++) {
-                        Cx v[T];
-#pragma unroll
-                        for (int i = 0; i < T; i++) v[i] = lds_cx(zp + (i * 3 + b) * 64);
-                        if (b == 2) {
-                            __syncwarp();
-                            if (lane == 0 && !dry) mbar_arrive(&zempty[zslot]);
-                        }
-#pragma unroll
-                        for (int i = 0; i < T; i++) cfma3<Real, Cx>(acc[i], u[b], v[i]);
-                    }
-                }
-                // xp operand of the epilogue: a ninth stage of the z/t ring (the producer copies the tile of xp behind
-                // the eight neighbour stages), so no arithmetic warp ever waits on global memory.  (With 3 T plain loads
-                // here the second half of M ran 1.83 ms against 1.38 ms for the bare stencil.)
-                const int zsx = npt * tc + 8, zslotx = zsx & (NZ - 1);
-                const Cx *zpx = reinterpret_cast<const Cx *>(zt + (size_t)zslotx * ZSTAGE) + j0 * 3 * 64 + sl;
-                if (XP && !dry) mbar_wait(&zfull[zslotx], (zsx >> nzlog) & 1);
-                if (!dry) mbar_wait_mem(redfull, tc & 1);
-#pragma unroll
-                for (int i = 0; i < T; i++) {
-#pragma unroll
-                    for (int cc = 0; cc < 3; cc++) {
-                        const Cx rb = red[((j0 + i) * 3 + cc) * 64 + sl];
-                        Cx o;
-                        o.x = acc[i][2 * cc] + rb.x;
-                        o.y = acc[i][2 * cc + 1] + rb.y;
+                        o.x = mx + shfl_x16(sx);
+                        o.y = my + shfl_x16(sy);
                         if (XP) {
-                            const Cx xv = lds_cx(zpx + (i * 3 + cc) * 64);
-                            o.x = fma((Real)p.a, xv.x, -o.x);
-                            o.y = fma((Real)p.a, xv.y, -o.y);
+                            o.x = fma((Real)p.a, xv[i][cc].x, -o.x);
+                            o.y = fma((Real)p.a, xv[i][cc].y, -o.y);
                         }
-                        if (jg + i < p.N) __stcs(vout + (size_t)(i * 3 + cc) * Vh, o);
+                        if (jg + io + i < p.N) __stcs(vout + (size_t)(i * 3 + cc) * Vh, o);
                     }
                 }
-                if (!dry) mbar_arrive_mem(redempty);
-                __syncwarp();
-                if (XP && lane == 0 && !dry) mbar_arrive(&zempty[zslotx]);
             }
         }
     }
@@ -547,60 +595,40 @@ static int build_segments(bkr_ctx *ctx, int N, int prec, int seglen)
 
 static const size_t WIN_SMEM_MAX = 232448;
 // returns 1 if this instantiation cannot run the geometry (caller falls back), BKR_OK after a launch, else an error
-template <typename Real, int T, int G, int C, bool XP>
+template <typename Real, int T, int C, bool XP>
 static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *in, void *out, const void *xp, double a,
                         const int *done)
 {
     typedef typename CxT<Real>::type Cx;
-    constexpr int NC = T * G;
+    constexpr int NC = 2 * T;
     const Geom &g = ctx->g;
     const int Xh = g.X[0] / 2;
     WinParams p;
     memset(&p, 0, sizeof(p));
     p.HcL = (3 * Xh + WIN_CHUNK - 1) / WIN_CHUNK;
-    {
-        const char *e = getenv("BKR_WIN_SLIM");
-        p.slim = e ? atoi(e) : 1;
-    }
+    p.slim = ctx->tune[BKR_TUNE_WIN_SLIM] == 2 ? 0 : 1;
     p.xover = (64 % Xh) != 0 ? 1 : 0;
     p.WCH = 2 * p.HcL + 2 + (p.slim ? std::max(0, 2 - (p.HcL - p.xover)) : 2);
     if (p.WCH > 16) return 1;
-    const size_t lstage = (size_t)9 * 64 * sizeof(Cx), wbytes = (size_t)p.WCH * NC * 3 * WIN_CHUNK * sizeof(Cx),
-                 zstage = (size_t)NC * 3 * 64 * sizeof(Cx), rbytes = (size_t)NC * 3 * 64 * sizeof(Cx), bbytes = 66 * 8;
-    // ring depths: as much data in flight as the 227 KB allow (the rings are what hides the ~1 us refill round trip);
-    // measured at 32^3 x 64, N = 8: 4 link stages + 2 z/t hop stages 0.69 ms; 8 + 2: 0.72; 4 + 3: 0.74 -- deeper rings do
-    // not help, the shared-memory port does the limiting
-    const char *zenv = getenv("BKR_WIN_NZ"), *lenv = getenv("BKR_WIN_RL");
-    int rl = lenv ? atoi(lenv) : 8, nz = zenv ? atoi(zenv) : 2;
-    if (rl != 4 && rl != 8) rl = 8;
-    if (nz != 1 && nz != 2 && nz != 4) nz = 2;
-    while (rl * lstage + wbytes + nz * zstage + rbytes + bbytes > WIN_SMEM_MAX) {
-        if (nz > 2) nz /= 2;
-        else if (rl > 4) rl = 4;
-        else if (nz > 1) nz /= 2;
-        else return 1;
-    }
-    {
-        // clusters of 3-4 CTAs need the deep link ring (the release -> refill round trip crosses SMs): with 4 stages the
-        // plain kernel is faster (48^3 x 96, N = 32 fp64: 20.6 vs 19.1 ms), with 8 it is not (32^3 x 64: 3.02 vs 3.10 ms)
-        if (C >= 3 && rl < 8 && ctx->dslash_force != 1) return 1;
-    }
-    if (nz < 2 && !getenv("BKR_WIN_ALLOW_NZ1")) return 1; // one z/t stage: slower than dslash.cu (48^4: 2.6 vs 2.1 ms)
-    p.nzlog = nz == 4 ? 2 : nz == 2 ? 1 : 0;
-    p.rllog = rl == 8 ? 3 : 2;
-    const size_t lbytes = rl * lstage;
-    p.off_win = (uint32_t)lbytes;
-    p.off_zt = (uint32_t)(lbytes + wbytes);
-    p.off_red = (uint32_t)(p.off_zt + nz * zstage);
-    p.off_bar = (uint32_t)(p.off_red + rbytes);
+    const size_t lstage = (size_t)9 * 64 * sizeof(Cx), wchunk = (size_t)NC * 3 * WIN_CHUNK * sizeof(Cx), wbytes = (size_t)p.WCH * wchunk,
+                 hstage = 2 * lstage + 2 * wchunk, bbytes = 64 * 8;
+    // Ring depth: what decides whether the arithmetic warps wait is how far ahead of its use a stage can be requested
+    // (a TMA round trip is 1300-2500 cycles on the loaded chip, a hop ~850 at the target rate; a slot is released a third of
+    // the way into the hop that reads it, so a ring of D stages gives D - 1/3 hops of lead).
+    int D = ctx->tune[BKR_TUNE_WIN_STAGES] ? ctx->tune[BKR_TUNE_WIN_STAGES] : 4;
+    D = std::min(D, 8);
+    while (D >= 2 && D * hstage + wbytes + bbytes > WIN_SMEM_MAX) D--;
+    if (D < 2) return 1;
+    // clusters of 3-4 CTAs need at least 3 stages (the release -> refill round trip crosses SMs)
+    if (C >= 3 && D < 3 && ctx->dslash_force != 1) return 1;
+    p.D = D;
+    p.off_win = (uint32_t)(D * hstage);
+    p.off_bar = (uint32_t)(p.off_win + wbytes);
     const size_t smem = p.off_bar + bbytes;
 
-    const char *senv = getenv("BKR_WIN_SEGLEN");
-    BKR_TRY(build_segments(ctx, N, prec, senv ? std::max(1, atoi(senv)) : 8));
-    CUtensorMap tm_win, tm_zt, tm_xp;
-    if (!make_map(&tm_win, in, prec, g.Vh, N, WIN_CHUNK, 3, NC) || !make_map(&tm_zt, in, prec, g.Vh, N, 64, 3, NC) ||
-        !make_map(&tm_xp, xp ? xp : in, prec, g.Vh, N, 64, 3, NC))
-        return 1;
+    BKR_TRY(build_segments(ctx, N, prec, ctx->tune[BKR_TUNE_WIN_SEGLEN] > 0 ? ctx->tune[BKR_TUNE_WIN_SEGLEN] : 8));
+    CUtensorMap tm_win;
+    if (!make_map(&tm_win, in, prec, g.Vh, N, WIN_CHUNK, 3, NC)) return 1;
 
     const int ntiles = link_tiles(g);
     p.g = g;
@@ -613,12 +641,8 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     p.segs = ctx->win_segs;
     p.nseg = ctx->win_nseg;
     p.done = done;
-    {
-        const char *oenv = getenv("BKR_WIN_OPTS");
-        p.opts = oenv ? atoi(oenv) : 0;
-    }
 
-    auto kern = dslash_win_kernel<Real, T, G, C, XP>;
+    auto kern = dslash_win_kernel<Real, T, C, XP>;
     static int max_clusters = -1, attr_dev = -1; // per instantiation; the shared-memory opt-in is per device
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
@@ -627,7 +651,7 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     attr[0].val.clusterDim.x = C;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
-    cfg.blockDim = dim3((4 * G + 4) * 32);
+    cfg.blockDim = dim3(WIN_THREADS);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->stream;
     cfg.attrs = attr;
@@ -645,10 +669,8 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
         }
     }
     if (max_clusters == 0) return 1;
-    if (getenv("BKR_WIN_DEBUG"))
-        fprintf(stderr, "dslash_win: C=%d max_clusters=%d nseg=%d smem=%zu WCH=%d nz=%d rl=%d\n", C, max_clusters, p.nseg, smem, p.WCH, nz, rl);
     cfg.gridDim = dim3((unsigned)(std::min(max_clusters, p.nseg) * C));
-    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tm_win, tm_zt, tm_xp, p);
+    cudaError_t e = cudaLaunchKernelEx(&cfg, kern, tm_win, p);
     if (e != cudaSuccess) {
         ctx->last_cuda = (int)e;
         return BKR_ECUDA;
@@ -656,12 +678,12 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     return bkr_check_launch(ctx);
 }
 
-template <typename Real, int T, int G, int C>
+template <typename Real, int T, int C>
 static int launch_win_c(bkr_ctx *ctx, int parity, int N, int prec, const void *in, void *out, const void *xp, double a,
                         const int *done)
 {
-    if (xp) return launch_win_x<Real, T, G, C, true>(ctx, parity, N, prec, in, out, xp, a, done);
-    return launch_win_x<Real, T, G, C, false>(ctx, parity, N, prec, in, out, xp, a, done);
+    if (xp) return launch_win_x<Real, T, C, true>(ctx, parity, N, prec, in, out, xp, a, done);
+    return launch_win_x<Real, T, C, false>(ctx, parity, N, prec, in, out, xp, a, done);
 }
 
 // 1 = not applicable (caller uses dslash.cu's kernel)
@@ -678,19 +700,15 @@ int launch_dslash_win(bkr_ctx *ctx, int out_parity, int N, int prec, const void 
     if (prec == BKR_F64) {
         const int C = (N + 7) / 8;
         if (mode == 1 && (N < 7 || 8 * C - N > 2)) return 1;
-        if (getenv("BKR_WIN_T8")) { // tuning probe
-            if (C == 1) return launch_win_c<double, 8, 1, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
-            if (C == 2) return launch_win_c<double, 8, 1, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
-        }
-        if (C == 1) return launch_win_c<double, 4, 2, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
-        if (C == 2) return launch_win_c<double, 4, 2, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
-        if (C == 3) return launch_win_c<double, 4, 2, 3>(ctx, out_parity, N, prec, in, out, xp, a, done);
-        if (C == 4) return launch_win_c<double, 4, 2, 4>(ctx, out_parity, N, prec, in, out, xp, a, done);
+        if (C == 1) return launch_win_c<double, 4, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
+        if (C == 2) return launch_win_c<double, 4, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
+        if (C == 3) return launch_win_c<double, 4, 3>(ctx, out_parity, N, prec, in, out, xp, a, done);
+        if (C == 4) return launch_win_c<double, 4, 4>(ctx, out_parity, N, prec, in, out, xp, a, done);
         return 1;
     }
     const int C = (N + 15) / 16;
     if (mode == 1 && (N < 13 || 16 * C - N > 3)) return 1;
-    if (C == 1) return launch_win_c<float, 8, 2, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
-    if (C == 2) return launch_win_c<float, 8, 2, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
+    if (C == 1) return launch_win_c<float, 8, 1>(ctx, out_parity, N, prec, in, out, xp, a, done);
+    if (C == 2) return launch_win_c<float, 8, 2>(ctx, out_parity, N, prec, in, out, xp, a, done);
     return 1;
 }

@@ -85,8 +85,6 @@ static RingPlan plan_ring(size_t L, size_t fixed, int min_stages, int nchunk_a, 
     RingPlan best;
     memset(&best, 0, sizeof(best));
     fixed = (fixed + 127) / 128 * 128;
-    static const char *renv = getenv("BKR_MB_R"); // tuning hook: force the rows per stage
-    const int rforce = renv ? atoi(renv) : 0;
     for (int R = 1024; R >= 64; R /= 2) {
         RingPlan p;
         p.R = R;
@@ -100,7 +98,6 @@ static RingPlan plan_ring(size_t L, size_t fixed, int min_stages, int nchunk_a, 
         p.nstg = n;
         p.smem = fixed + (size_t)n * p.stage_bytes;
         bool ok = n >= min_stages && (L + R - 1) / R >= (size_t)2 * BKR_NUM_SMS;
-        if (rforce) ok = R == rforce && n >= 2;
         if (ok || R == 64) {
             if (n < 2) p.nstg = 0; // does not fit at all (cannot happen for N <= 32)
             best = p;
