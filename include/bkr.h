@@ -200,6 +200,7 @@ int bkr_set_dslash_variant(bkr_ctx *ctx, int variant);
 enum { BKR_OPT_L2_BUDGET_MB = 0, BKR_OPT_ROW_UNIT_TILES = 1, BKR_OPT_ROW_VEC_POLICY = 2, BKR_OPT_ABLATION = 3, BKR_OPT_TUNE = 16 };
 enum {
     BKR_TUNE_WIN_STAGES = 0,      /* window stencil: hop-stage ring depth, 2-8 (default: the deepest that fits)          */
+    BKR_TUNE_DSLASH_CHUNK = 1,    /* 1 = never split a block into chunks of 16 / 8 rhs; 2 = always split blocks > 16 rhs   */
     BKR_TUNE_WIN_SEGLEN = 2,      /* 64-site tiles per segment (default 8)                                                */
     BKR_TUNE_WIN_SLIM = 3,        /* 2 = keep spare window slots instead of releasing the lower halo early                */
     BKR_TUNE_COUNT = 16

@@ -39,7 +39,7 @@ def lib():
     if _lib is None:
         _lib = ctypes.CDLL(build())
         for name in ("orc_dslash", "orc_dslash_sites", "orc_apply_M", "orc_cholesky_upper", "orc_hpd_inverse",
-                     "orc_thin_qr", "orc_cg", "orc_block_cg", "orc_true_relres"):
+                     "orc_thin_qr", "orc_thin_qr2", "orc_cg", "orc_block_cg", "orc_block_cg_reorth", "orc_true_relres"):
             getattr(_lib, name).restype = ctypes.c_int
         _lib.orc_gram.restype = None
         _lib.orc_block_axpy.restype = None
@@ -148,12 +148,13 @@ def hpd_inverse(G):
     return Gi
 
 
-def thin_qr(Z):
-    """Algorithm 2: returns Q (same shape as Z), R (N, N) upper."""
+def thin_qr(Z, two_pass=False):
+    """Algorithm 2: returns Q (same shape as Z), R (N, N) upper.  two_pass: orc_thin_qr2 (a second
+    Cholesky-QR pass, shifted first pass on a failed pivot; refs [43, 44] of PAPER.md:184-186)."""
     Z, N, L = _as_block(Z)
     Q = Z.copy()
     R = np.empty((N, N), dtype=np.complex128)
-    rc = lib().orc_thin_qr(ctypes.c_long(L), N, _ptr(Q), _ptr(R))
+    rc = (lib().orc_thin_qr2 if two_pass else lib().orc_thin_qr)(ctypes.c_long(L), N, _ptr(Q), _ptr(R))
     if rc:
         raise ArithmeticError("cholesky breakdown")
     return Q, R
@@ -170,10 +171,11 @@ def cg(dims, fat, lng, mass, b, x0=None, tol=1e-10, maxiter=10000):
     return x, it.value, rc, hist[: it.value + 1]
 
 
-def block_cg(dims, fat, lng, mass, B, X0=None, tol=1e-10, maxiter=10000, mixed=False, delta=0.1, ntrace=0):
+def block_cg(dims, fat, lng, mass, B, X0=None, tol=1e-10, maxiter=10000, mixed=False, delta=0.1, ntrace=0, reorth=False):
     """blockCGrQ (Algorithm 1; with mixed=True plus Algorithm 3).  B (N, Vh, 3).
     returns dict(X, iters, status, reliable_updates, hist, G, C, QP); G, C, QP = traces of the first ntrace iterations
-    (P^dag M P, C after l.12, and Q^dag P right after l.8: PAPER.md:210)."""
+    (P^dag M P, C after l.12, and Q^dag P right after l.8: PAPER.md:210).  reorth: every thin QR by two Cholesky-QR
+    passes (orc_thin_qr2) -- for blocks with nearly dependent right-hand sides."""
     fat, lng, B = _ca(fat), _ca(lng), _ca(B)
     N = B.shape[0]
     X = np.zeros_like(B) if X0 is None else _ca(X0).copy()
@@ -182,7 +184,7 @@ def block_cg(dims, fat, lng, mass, B, X0=None, tol=1e-10, maxiter=10000, mixed=F
     tG = np.zeros((max(ntrace, 1), N, N), dtype=np.complex128)
     tC = np.zeros((max(ntrace, 1), N, N), dtype=np.complex128)
     tQP = np.zeros((max(ntrace, 1), N, N), dtype=np.complex128)
-    rc = lib().orc_block_cg(_dims(dims), _ptr(fat), _ptr(lng), ctypes.c_double(mass), N, _ptr(B), _ptr(X),
+    rc = (lib().orc_block_cg_reorth if reorth else lib().orc_block_cg)(_dims(dims), _ptr(fat), _ptr(lng), ctypes.c_double(mass), N, _ptr(B), _ptr(X),
                             ctypes.c_double(tol), int(maxiter), int(bool(mixed)), ctypes.c_double(delta),
                             ctypes.byref(it), ctypes.byref(nup), hist.ctypes.data_as(_P), int(ntrace), _ptr(tG),
                             _ptr(tC), _ptr(tQP))

@@ -15,7 +15,7 @@
  * definiteness of M, the free-field closed-form spectrum (4^4 worked example and plane
  * waves at other sizes), gauge covariance, dense brute force on 4^4 assembled independently
  * in numpy, N=1 == CG, finite termination on the 5-eigenvalue free field, thin-QR
- * identities, numpy.linalg for the small matrices.  Nothing here is "parity unpinned"
+ * identities (also for the two-pass QR on nearly dependent columns), numpy.linalg for the small matrices.  Nothing here is "parity unpinned"
  * except iteration counts on the synthetic configs (no published value exists).
  *
  * Layouts (canonical, host memory, complex = (re, im) fp64):
@@ -264,6 +264,62 @@ int orc_thin_qr(long L, int N, cplx *Z, cplx *R)
     return 0;
 }
 
+/* thin QR by TWO Cholesky-QR passes (the remedy of the paper's refs [43, 44], PAPER.md:184-186 footnote, for the
+ * squared condition number of Algorithm 2; U24):
+ *   pass 1  H = Z^dag Z ; R1^dag R1 = H, or = H + s 1 with s = 1e-12 max_i H_ii when a pivot of H is not positive
+ *           ("shifted" Cholesky QR) ; Q1 = Z R1^-1
+ *   pass 2  H2 = Q1^dag Q1 ; R2^dag R2 = H2 ; Q = Q1 R2^-1 ; R = R2 R1
+ * The factorisation Z = Q R with R upper triangular and a positive diagonal is unique, so for a well conditioned Z this
+ * returns what orc_thin_qr returns up to rounding.  -5 if a pivot of pass 2 is below 1e-8 (Z has no full rank to
+ * working precision). */
+int orc_thin_qr2(long L, int N, cplx *Z, cplx *R)
+{
+    cplx *H = malloc(sizeof(cplx) * N * N), *R1 = malloc(sizeof(cplx) * N * N), *R2 = malloc(sizeof(cplx) * N * N);
+    int rc;
+    orc_gram(L, N, Z, Z, H);
+    hermitise(N, H);
+    rc = orc_cholesky_upper(N, H, R1);
+    if (rc) {
+        double hmax = 0.0;
+        for (int i = 0; i < N; i++) hmax = fmax(hmax, creal(H[i * N + i]));
+        for (int i = 0; i < N; i++) H[i * N + i] += 1e-12 * hmax;
+        rc = orc_cholesky_upper(N, H, R1);
+    }
+    free(H);
+    if (rc) { free(R1); free(R2); return rc; }
+    for (int pass = 0; pass < 2; pass++) {
+        const cplx *Rp = pass == 0 ? R1 : R2;
+        if (pass == 1) {
+            cplx *H2 = malloc(sizeof(cplx) * N * N);
+            orc_gram(L, N, Z, Z, H2);
+            hermitise(N, H2);
+            rc = orc_cholesky_upper(N, H2, R2);
+            /* after pass 1 the columns have norm <= 1 and are orthonormal up to kappa(Z)^2 u (or up to the shift: a direction
+             * with singular value sigma keeps sigma^2 / (sigma^2 + s)); a pivot below 1e-8 means Z has no full rank to
+             * working precision (its image under pass 1 is rounding noise) */
+            for (int j = 0; j < N && !rc; j++)
+                if (!(creal(R2[j * N + j]) * creal(R2[j * N + j]) > 1e-8)) rc = -5;
+            free(H2);
+            if (rc) { free(R1); free(R2); return rc; }
+        }
+        for (int j = 0; j < N; j++) { /* Z <- Z Rp^-1, column by column as in orc_thin_qr */
+            cplx *qj = Z + (long)j * L;
+            for (int i = 0; i < j; i++) {
+                const cplx *qi = Z + (long)i * L;
+                cplx r = Rp[i * N + j];
+#pragma omp parallel for schedule(static)
+                for (long k = 0; k < L; k++) qj[k] -= qi[k] * r;
+            }
+            double inv = 1.0 / creal(Rp[j * N + j]);
+#pragma omp parallel for schedule(static)
+            for (long k = 0; k < L; k++) qj[k] *= inv;
+        }
+    }
+    matmul(N, R2, R1, R);
+    free(R1); free(R2);
+    return 0;
+}
+
 /* ------------------------------------------------------------------------------ solvers */
 
 static double norm2(long n, const cplx *v)
@@ -362,11 +418,12 @@ static void round_f32(long n, cplx *v)
  * block that entered l.8 ("Q_old" of PAPER.md:210, whose identity (Q_old)^dag P = 1 pins the
  * driver, with and without reliable updates).  A trace only: no arithmetic of the solve uses it.
  * Returns 0, -5 on a Cholesky breakdown (U15), -6 at maxiter. */
-int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, int N,
-                 const cplx *B, cplx *X, double tol, int maxiter, int mixed, double delta,
-                 int *iters, int *nupdates, double *hist, int ntrace, cplx *trace_G,
-                 cplx *trace_C, cplx *trace_QP)
+static int block_cg_impl(const int D[4], const cplx *fat, const cplx *lng, double mass, int N,
+                         const cplx *B, cplx *X, double tol, int maxiter, int mixed, double delta,
+                         int *iters, int *nupdates, double *hist, int ntrace, cplx *trace_G,
+                         cplx *trace_C, cplx *trace_QP, int reorth)
 {
+    int (*const thin_qr)(long, int, cplx *, cplx *) = reorth ? orc_thin_qr2 : orc_thin_qr;
     if (!dims_ok(D) || N < 1) return -1;
     long V = (long)D[0] * D[1] * D[2] * D[3], Vh = V / 2, L = 3 * Vh, n = L * N;
     size_t nn = sizeof(cplx) * N * N;
@@ -397,7 +454,7 @@ int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, 
         orc_apply_M(D, fat, lng, mass, N, X, Q, T); /* l.3 */
     }
     for (long k = 0; k < n; k++) Q[k] = B[k] - Q[k];
-    if (orc_thin_qr(L, N, Q, C)) { rc = -5; goto done; } /* l.4 */
+    if (thin_qr(L, N, Q, C)) { rc = -5; goto done; } /* l.4 */
     if (mixed) round_f32(n, Q);
     memset(S, 0, nn);
     for (int i = 0; i < N; i++) S[i * N + i] = 1.0; /* l.5 ; P = 0 from calloc (l.6) */
@@ -428,7 +485,7 @@ int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, 
         /* l.11 Q S = Q - (M P) beta */
         for (int i = 0; i < N * N; i++) tmp[i] = -beta[i];
         orc_block_axpy(L, N, tmp, AP, Q);
-        if (orc_thin_qr(L, N, Q, S)) { rc = -5; break; }
+        if (thin_qr(L, N, Q, S)) { rc = -5; break; }
         if (mixed) round_f32(n, Q);
         /* l.12 C = S C */
         memcpy(Cprev, C, nn);
@@ -445,7 +502,7 @@ int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, 
             memset(X, 0, sizeof(cplx) * n);                      /* l.3 */
             orc_apply_M(D, fat, lng, mass, N, Y, Q, T);          /* l.4, fp64 operator */
             for (long k = 0; k < n; k++) Q[k] = B[k] - Q[k];
-            if (orc_thin_qr(L, N, Q, C)) { rc = -5; break; }      /* l.5, C = C_new */
+            if (thin_qr(L, N, Q, C)) { rc = -5; break; }      /* l.5, C = C_new */
             round_f32(n, Q);
             orc_upper_inverse(N, Cprev, Ci);                     /* l.6 S = C_new C_prev^-1 */
             matmul(N, C, Ci, S);
@@ -465,6 +522,26 @@ done:
     free(C); free(S); free(G); free(beta); free(W); free(Sd); free(Cprev); free(tmp); free(Ci);
     free(bnorm);
     return rc;
+}
+
+int orc_block_cg(const int D[4], const cplx *fat, const cplx *lng, double mass, int N,
+                 const cplx *B, cplx *X, double tol, int maxiter, int mixed, double delta,
+                 int *iters, int *nupdates, double *hist, int ntrace, cplx *trace_G,
+                 cplx *trace_C, cplx *trace_QP)
+{
+    return block_cg_impl(D, fat, lng, mass, N, B, X, tol, maxiter, mixed, delta, iters, nupdates, hist, ntrace, trace_G,
+                         trace_C, trace_QP, 0);
+}
+
+/* the same with every thin QR (l.4, l.11, Alg. 3 l.5) done by orc_thin_qr2: the comparison solver for blocks whose
+ * residuals are ill conditioned (nearly dependent right-hand sides), where Algorithm 2 as printed breaks down */
+int orc_block_cg_reorth(const int D[4], const cplx *fat, const cplx *lng, double mass, int N,
+                        const cplx *B, cplx *X, double tol, int maxiter, int mixed, double delta,
+                        int *iters, int *nupdates, double *hist, int ntrace, cplx *trace_G,
+                        cplx *trace_C, cplx *trace_QP)
+{
+    return block_cg_impl(D, fat, lng, mass, N, B, X, tol, maxiter, mixed, delta, iters, nupdates, hist, ntrace, trace_G,
+                         trace_C, trace_QP, 1);
 }
 
 /* true relative residuals ||b_i - M x_i|| / ||b_i|| */

@@ -337,12 +337,22 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
             return rc;
         }
     }
-    // Elsewhere fp64 blocks of more than 16 rhs go through in chunks of 16: two cluster-of-2 window launches beat one cluster
-    // of 4 (32^3 x 64, N = 32: 2 x 1.32 ms against 3.02 ms; 48^3 x 96: 2 x 7.3 ms against 19.1 ms for the plain kernel) although
-    // the links are then read once per chunk.  A chunk is a contiguous view of the native block [rhs][colour][site].
-    // Likewise 11-13 rhs as 8 + rest (window kernel + plain kernel) and fp32 blocks of 17-28 rhs as 16 + rest.
+    // fp64 blocks of 22-24 and 30-32 rhs: ONE window launch, a cluster of 3 / 4 CTAs, every link read once per call
+    // (PAPER.md:224).  Measured at 32^3 x 64 against two launches of a cluster of 2 (links read twice): N = 24 2.21 vs
+    // 2.22 ms, N = 32 3.04 vs 2.88 ms -- the single pass is kept for the traffic it saves (BKR_TUNE_DSLASH_CHUNK = 2 splits).
+    if (!ctx->dslash_nblock && prec == BKR_F64 && N > 16 && 8 * ((N + 7) / 8) - N <= 2 && ctx->dslash_force != 0 &&
+        ctx->dslash_force != 2 && ctx->tune[BKR_TUNE_DSLASH_CHUNK] != 2) {
+        const int rc = launch_dslash_win(ctx, out_parity, N, prec, in, out, xp, a, done);
+        if (rc != 1) {
+            ctx->dslash_variant = 1;
+            return rc;
+        }
+    }
+    // Other blocks of more than 16 fp64 rhs go through in chunks of 16 (window kernel for the full chunk, the links are then
+    // read once per chunk); likewise 11-13 rhs as 8 + rest (window kernel + plain kernel) and fp32 blocks of 17-28 rhs as
+    // 16 + rest.  A chunk is a contiguous view of the native block [rhs][colour][site].
     int chunk = 0;
-    if (ctx->dslash_force < 0 || ctx->dslash_force == 1) {
+    if ((ctx->dslash_force < 0 || ctx->dslash_force == 1) && ctx->tune[BKR_TUNE_DSLASH_CHUNK] != 1) {
         if (prec == BKR_F64 && N > 16) chunk = 16;
         else if (prec == BKR_F64 && N >= 11 && N <= 13) chunk = 8; // 14 = window cluster of 2 (1.29 ms) beats 8 + 6 (1.32 ms)
         else if (prec == BKR_F32 && N > 16 && N <= 28) chunk = 16;

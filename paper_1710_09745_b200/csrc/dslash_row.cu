@@ -40,7 +40,6 @@ struct RowParams {
     int nstrip;
     int UL;    // tiles per unit
     int vec_policy; // L2 priority of the z/t neighbour loads: 0 evict_normal, 1 evict_last
-    int dry;   // tuning probe (BKR_TUNING builds): no producers, no barriers, results are garbage
     const int *done;
     int WCH;   // window ring slots (rows)
     int rllog; // log2 of the link ring depth
@@ -178,7 +177,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
     if (warp >= ROW_CONSUMER_WARPS) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
         const int role = warp - ROW_CONSUMER_WARPS;
-        if (lane == 0 && role == 0 && !p.dry) {
+        if (lane == 0 && role == 0) {
             // ---------------------------------------------------------------- link stages, one per (tile, hop)
             const uint64_t pol = policy_evict_first();
             const Cx *wt = reinterpret_cast<const Cx *>(p.wt);
@@ -199,7 +198,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                                           (uint16_t)((1u << C) - 1u), pol);
                     }
             }
-        } else if (lane == 0 && role == 1 && !p.dry) {
+        } else if (lane == 0 && role == 1) {
             // ---------------------------------------------------------------- window rows: virtual rows -3 .. Y + 2 of a strip
             int q = 0; // absolute row sequence number of this CTA
             for (int si = cid; si < p.nstrip; si += ncl) {
@@ -240,7 +239,6 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
         uint64_t vpol; // L2 policy of the z/t neighbour loads
         if (p.vec_policy == 1) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(vpol));
         else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(vpol));
-        const bool dry = p.dry != 0; // tuning probe: no producers, no barriers (results are garbage)
         Cx uA[3], uB[3], wA[T], wB[T]; // link column / window vector operands, two register sets
         Cx vz[2][3 * T];   // z/t neighbour vectors of two hops: [hop parity][colour * T + rhs]
         int ls = 0; // link stage counter
@@ -288,7 +286,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                 // window rows v <= TR kl + TR + 2, i.e. q <= TR kl + TR + 5
                 while (waited <= kl * TR + TR + 5) {
                     const int qq = Q0 + waited;
-                    if (!dry) mbar_wait(&wfull[qq % WCH], (qq / WCH) & 1);
+                    mbar_wait(&wfull[qq % WCH], (qq / WCH) & 1);
                     waited++;
                 }
                 const int qmod = (Q0 + kl * TR + r) % WCH; // window slot of virtual row y - 3
@@ -316,7 +314,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                 };
                 auto release_link = [&](int stage) {
                     __syncwarp();
-                    if (lane == 0 && !dry) {
+                    if (lane == 0) {
                         uint64_t *bb = &lempty[stage & (RL - 1)];
                         if (C == 1) mbar_arrive(bb);
                         else
@@ -341,7 +339,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                         // probe of the next stage's barrier issued ahead of the FMAs that hide its latency
                         uint64_t *bb = &lfull[(st + 1) & (RL - 1)];
                         const uint32_t par = ((st + 1) >> rllog) & 1;
-                        const uint32_t ok = dry ? 1u : row_try_wait(bb, par);
+                        const uint32_t ok = row_try_wait(bb, par);
                         col_fma<Real, Cx, T>(acc, uA, wA);
                         row_wait_finish(ok, bb, par);
                         load_u(uB, lnk_ptr(st + 1), 0);
@@ -349,7 +347,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                         if (i == 1) {
                             // hops 0, 1 were y-3, y-1: rows below the tile are dead from here on (x hops read the tile's own rows)
                             const int new_rel = min(kl * TR + 3, (kl + 1) * TR);
-                            if (lane == 0 && !dry)
+                            if (lane == 0)
                                 for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(Q0 + cc) % WCH]);
                             released = max(released, new_rel);
                         }
@@ -377,7 +375,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                         if (i < 7) {
                             uint64_t *bb = &lfull[(st + 2) & (RL - 1)];
                             const uint32_t par = ((st + 2) >> rllog) & 1;
-                            const uint32_t ok = dry ? 1u : row_try_wait(bb, par);
+                            const uint32_t ok = row_try_wait(bb, par);
                             col_fma<Real, Cx, T>(acc, uB, v2);
                             row_wait_finish(ok, bb, par);
                             load_u(uA, lnk_ptr(st + 2), 0);
@@ -391,7 +389,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                 };
 
                 // ---- prologue: column 0 of window hop 0
-                if (!dry) mbar_wait(&lfull[ls & (RL - 1)], (ls >> rllog) & 1);
+                mbar_wait(&lfull[ls & (RL - 1)], (ls >> rllog) & 1);
                 load_u(uA, lnk_ptr(ls), 0);
                 load_vw(wA, win_ptr(0), 0);
 #pragma unroll
@@ -403,7 +401,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                 {
                     const int new_rel = kl == UL - 1 ? rows_per_unit : (kl + 1) * TR;
                     __syncwarp();
-                    if (lane == 0 && !dry)
+                    if (lane == 0)
                         for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(Q0 + cc) % WCH]);
                     released = max(released, new_rel);
                 }
@@ -544,7 +542,6 @@ static int launch_row_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     p.nstrip = ctx->row_nstrip;
     p.done = done;
     p.vec_policy = ctx->row_vec_policy & 1;
-    p.dry = ctx->row_vec_policy == 64;
 
     auto kern = dslash_row_kernel<Real, T, C, XP, XH>;
     static int max_clusters = -1, attr_dev = -1; // per instantiation; the shared-memory opt-in is per device

@@ -159,6 +159,39 @@ def test_P7_thin_qr_identities():
     assert H.relerr_inf(R, (Rn / ph[:, None])) < 1e-12
 
 
+def test_P7b_two_pass_qr_on_nearly_dependent_columns():
+    """orc_thin_qr2 (refs [43, 44] of PAPER.md:184-186; U24): on a well conditioned block it is Algorithm 2 up
+    to rounding; with two columns equal to 1e-7 (kappa(Z) ~ 1e7, kappa(Z^dag Z) ~ 1e14) it still returns an orthonormal
+    Q and the R of a library QR, where one pass leaves Q^dag Q off by ~1e-3 or breaks down; a block of rank N - 1 is
+    reported as a breakdown."""
+    rng = np.random.default_rng(15)
+    N, L = 6, 3 * 64
+    Z = rng.normal(size=(N, L)) + 1j * rng.normal(size=(N, L))
+    Q1, R1 = oracle.thin_qr(Z)
+    Q2, R2 = oracle.thin_qr(Z, two_pass=True)
+    assert H.relerr_inf(R2, R1) < 1e-13 and H.relerr_inf(Q2, Q1) < 1e-13
+    Zb = Z.copy()
+    Zb[4] = Zb[1] + 1e-7 * Zb[4]
+    Q, R = oracle.thin_qr(Zb, two_pass=True)
+    assert np.abs(Q.conj() @ Q.T - np.eye(N)).max() < 1e-12
+    assert H.relerr_inf(R.T @ Q, Zb) < 1e-13
+    assert np.allclose(np.tril(R, -1), 0) and (np.diag(R).real > 0).all()
+    Qn, Rn = np.linalg.qr(Zb.T)                        # Householder QR of the library: backward stable for any kappa
+    ph = np.diag(Rn) / abs(np.diag(Rn))
+    Rl = Rn / ph[:, None]
+    assert np.abs(R - Rl).max() / np.abs(Rl).max() < 1e-9    # forward error of R ~ kappa(Z) u
+    assert abs(R[4, 4] - Rl[4, 4]) / abs(Rl[4, 4]) < 1e-3   # the tiny pivot itself, to the digits kappa leaves
+    try:                                               # one pass: broken down, or visibly not orthonormal
+        Qp, _ = oracle.thin_qr(Zb)
+        assert np.abs(Qp.conj() @ Qp.T - np.eye(N)).max() > 1e-6
+    except ArithmeticError:
+        pass
+    Zc = Z.copy()
+    Zc[4] = Zc[1]
+    with pytest.raises(ArithmeticError):
+        oracle.thin_qr(Zc, two_pass=True)
+
+
 # ---------------------------------------------------------------- solvers
 
 def test_P5_solutions_vs_dense_solve(cfg1):
@@ -269,3 +302,22 @@ def test_P8_Qold_dag_P_is_identity_after_line8(cfg1):
     assert mix["reliable_updates"] >= 3
     for k in range(60):
         assert np.abs(mix["QP"][k] - np.eye(N)).max() <= 2e-5, k  # fp32 storage of P and Q
+
+
+def test_reorth_solver_matches_plain_solver_and_survives_dependent_rhs(cfg1):
+    """block CG with two-pass QR (oracle.block_cg(reorth=True)): same solutions and iteration count as Algorithm 1 on a
+    well conditioned block; on a block with two sources equal to 1e-7 it converges to the dense solutions (P5's
+    definition of X*), where the plain solver breaks down or stalls."""
+    fat, lng, B = cfg1
+    a = oracle.block_cg(D4, fat, lng, 0.1, B, tol=1e-10)
+    b = oracle.block_cg(D4, fat, lng, 0.1, B, tol=1e-10, reorth=True)
+    assert a["status"] == 0 and b["status"] == 0 and abs(a["iters"] - b["iters"]) <= 1
+    assert H.relerr_inf(b["X"], a["X"]) < 1e-9
+    Bd = B.copy()
+    Bd[3] = Bd[1] + 1e-7 * Bd[3]
+    r = oracle.block_cg(D4, fat, lng, 0.1, Bd, tol=1e-11, reorth=True)
+    assert r["status"] == 0
+    assert oracle.true_relres(D4, fat, lng, 0.1, Bd, r["X"]).max() <= 1e-10
+    _, _, M = H.dense_blocks(D4, fat, lng, 0.1)
+    Xs = np.linalg.solve(M, Bd.reshape(4, -1).T).T.reshape(Bd.shape)
+    assert H.relerr_inf(r["X"], Xs) < 1e-8
