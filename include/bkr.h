@@ -55,7 +55,8 @@ enum {
     BKR_ENOLINKS = -2,   /* operator call before bkr_load_links (or fp32 links not requested)      */
     BKR_ENOMEM = -3,     /* device or host allocation failed                                       */
     BKR_ECUDA = -4,      /* a CUDA call failed; bkr_last_cuda_error() gives the cudaError_t        */
-    BKR_EBREAKDOWN = -5, /* non-positive / non-finite Cholesky pivot; X = best so far */
+    BKR_EBREAKDOWN = -5, /* the block lost rank for good (two-pass QR included) or a Gram matrix is non-finite
+                          * (PAPER.md:109); X = best so far */
     BKR_ENOCONV = -6     /* maxiter reached; X holds the last iterate, stats are filled             */
 };
 
@@ -68,6 +69,7 @@ typedef struct {
     double true_relres_max; /* max_i ||b_i - M x_i|| / ||b_i||, recomputed in fp64          */
     double iter_relres_max; /* max_i ||C[:,i]|| / ||b_i|| the loop stopped on */
     long long gpu_launches; /* kernels launched by this call                                  */
+    int reorthonormalisations; /* two-pass QRs of an ill-conditioned residual block (refs [43, 44]) */
 } bkr_stats;
 
 /* Create a context for an X*Y*Z*T lattice on CUDA device `device`; `cuda_stream` is a cudaStream_t

@@ -30,7 +30,8 @@ SYMBOLS = (
 class Stats(ctypes.Structure):
     _fields_ = [("iters", ctypes.c_int), ("reliable_updates", ctypes.c_int), ("status", ctypes.c_int),
                 ("restarts", ctypes.c_int), ("seconds", ctypes.c_double), ("true_relres_max", ctypes.c_double),
-                ("iter_relres_max", ctypes.c_double), ("gpu_launches", ctypes.c_longlong)]
+                ("iter_relres_max", ctypes.c_double), ("gpu_launches", ctypes.c_longlong),
+                ("reorthonormalisations", ctypes.c_int)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

@@ -36,6 +36,8 @@ template <> struct CxT<float> { typedef float2 type; };
 struct SolverFlags {
     int done;          // 1: converged or broken down -> loop kernels become no-ops
     int breakdown;     // 1: non-positive / non-finite Cholesky pivot
+    int illcond;       // with breakdown: every entry was finite -- the block is (nearly) rank deficient, not broken: the host
+                       // restarts from X with the two-pass QR (solver.cu, PAPER.md:184-186 refs [43, 44])
     int iters;         // completed iterations (Alg. 1 l.9 applications of M)
     int want_update;   // mixed precision: reliable update requested (Alg. 3)
     double relres_max; // max_i ||C[:,i]|| / ||b_i||  after the last l.12
@@ -189,8 +191,9 @@ struct SmallArgs {
     SolverFlags *flags;
     int *status;             // API path
     int mixed;
+    double pivot_tol;        // breakdown when a pivot d <= pivot_tol * h_jj (0: the mode's default)
 };
-enum { SMALL_CHOL = 0, SMALL_HPDINV = 1, SMALL_BETA = 2, SMALL_QR = 3, SMALL_INIT = 4, SMALL_RELUPD = 5 };
+enum { SMALL_CHOL = 0, SMALL_HPDINV = 1, SMALL_BETA = 2, SMALL_QR = 3, SMALL_INIT = 4, SMALL_RELUPD = 5, SMALL_RQ1 = 6, SMALL_RQ2 = 7 };
 int launch_small(bkr_ctx *ctx, const SmallArgs &args);
 // CG scalar kernel: per-rhs alpha / beta / convergence bookkeeping
 struct CgScalars {

@@ -12,6 +12,10 @@
 //   SMALL_QR      l.11/l.12: H = sum partials; S = chol(H); Sinv; Sdag; Cprev = C; C = S C; residuals, flags
 //   SMALL_INIT    l.4-l.5:  H = sum partials; C = chol(H); Sinv = C^-1 (to form Q = R C^-1); Sdag = 1
 //   SMALL_RELUPD  Alg. 3 l.5-l.6: C_new = chol(H); Sinv = C_new^-1; Sdag = (C_new Cprev^-1)^dag; C = C_new
+//   SMALL_RQ1     two-pass QR of an ill-conditioned residual block (refs [43, 44] of PAPER.md:184-186), pass 1:
+//                 H = sum partials; R1 = chol(H + 1e-12 max_i H_ii); W = R1 (scratch); Sinv = R1^-1
+//   SMALL_RQ2     pass 2: H2 = sum partials; R2 = chol(H2), breakdown when a pivot is below 1e-8 (no full rank);
+//                 C = R2 R1; Sinv = R2^-1; then as SMALL_INIT
 #include "common.cuh"
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b)
@@ -29,13 +33,19 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 b) // conj(a) * b
 // Breakdown (U15): a pivot that is non-finite, non-positive, or has lost more than 13
 // digits against the diagonal entry it started from (d <= 1e-13 h_jj: the column is linearly dependent on the
 // previous ones to working precision, and only rounding noise decides the sign of the pivot).
-__device__ bool warp_cholesky_upper(int N, double2 *A, int lane)
+// rel_tol / abs_tol: a pivot must exceed rel_tol * h_jj and abs_tol.  *finite_out: no NaN / Inf was met.
+__device__ bool warp_cholesky_upper(int N, double2 *A, int lane, double rel_tol, double abs_tol, bool *finite_out)
 {
     const double h0 = lane < N ? A[lane * N + lane].x : 0.0;
+    *finite_out = true;
     for (int j = 0; j < N; j++) {
         double d = A[j * N + j].x;
         double hjj = __shfl_sync(0xffffffffu, h0, j);
-        if (!(d > 1e-13 * hjj) || !isfinite(d)) return false; // uniform across the warp
+        if (!isfinite(d) || !isfinite(hjj)) {
+            *finite_out = false;
+            return false;
+        }
+        if (!(d > rel_tol * hjj) || !(d > abs_tol)) return false; // uniform across the warp
         double rjj = sqrt(d);
         __syncwarp();
         if (lane < N) {
@@ -144,7 +154,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
     extern __shared__ double2 sm[];
     const int N = p.N, NN = N * N;
     double2 *A = sm, *B = sm + NN, *Cm = sm + 2 * NN, *Dm = sm + 3 * NN;
-    __shared__ int ok_s;
+    __shared__ int ok_s, finite_s;
     __shared__ double scratch[BKR_MAX_N];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     SolverFlags *fl = p.flags;
@@ -157,10 +167,26 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
     }
 
     load_hermitian(p, A);
+    if (p.mode == SMALL_RQ1) { // shifted Cholesky QR: H + s 1, s = 1e-12 max_i H_ii
+        double hmax = 0.0;
+        for (int i = 0; i < N; i++) hmax = fmax(hmax, A[i * N + i].x);
+        __syncthreads();
+        if (threadIdx.x < N) A[threadIdx.x * N + threadIdx.x].x += 1e-12 * hmax;
+        __syncthreads();
+    }
     if (warp == 0) {
-        bool ok = warp_cholesky_upper(N, A, lane); // A = R
+        // Breakdown thresholds (U15): 13 digits lost against the diagonal entry for Gram matrices of fp64 blocks;
+        // fp32 blocks carry rounding noise of ~1e-7 h_jj, so a rank-deficient one would pass that test with a noise pivot:
+        // the caller passes pivot_tol = 4e-6 there.  Pass 2 of the two-pass QR: columns have norm <= 1 after pass 1, a
+        // pivot below 1e-8 is the image of rounding noise (no full rank).
+        const double rel = p.pivot_tol > 0.0 ? p.pivot_tol : 1e-13;
+        bool fin = true;
+        bool ok = warp_cholesky_upper(N, A, lane, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin); // A = R
         if (ok) warp_upper_inverse(N, A, B, lane); // B = R^-1
-        if (lane == 0) ok_s = ok ? 1 : 0;
+        if (lane == 0) {
+            ok_s = ok ? 1 : 0;
+            finite_s = fin ? 1 : 0;
+        }
     }
     __syncthreads();
     const bool ok = ok_s != 0;
@@ -169,6 +195,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
             if (p.status) *p.status = BKR_EBREAKDOWN;
             if (fl) {
                 fl->breakdown = 1;
+                fl->illcond = (finite_s && p.mode != SMALL_RQ2) ? 1 : 0;
                 fl->done = 1;
                 if (p.mode == SMALL_BETA) {
                     fl->xpend = 0;
@@ -259,6 +286,30 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
         }
         break;
     }
+    case SMALL_RQ1:
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            p.W[o] = A[o];    // R1, kept for pass 2
+            p.Sinv[o] = B[o]; // Q1 = R R1^-1
+        }
+        break;
+    case SMALL_RQ2: // C = R2 R1 (both upper triangular), then as SMALL_INIT with A = C
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            Dm[o] = p.W[o];
+            Cm[o] = A[o];
+        }
+        __syncthreads();
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
+            int i = o / N, j = o % N;
+            double2 s = make_double2(0.0, 0.0);
+            for (int k = i; k <= j; k++) {
+                double2 t = cmul(Cm[i * N + k], Dm[k * N + j]);
+                s.x += t.x;
+                s.y += t.y;
+            }
+            A[o] = s;
+        }
+        __syncthreads();
+        // fall through
     case SMALL_INIT: {
         for (int o = threadIdx.x; o < NN; o += blockDim.x) {
             int i = o / N, j = o % N;

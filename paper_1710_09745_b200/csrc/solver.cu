@@ -13,6 +13,7 @@ struct Workspace {
     int N, prec;
     size_t bytes64, bytesP;
     double2 *Bn, *Xn, *Y, *R64;   // fp64 native blocks (Y, R64 only for the mixed solver; else R64 aliases AP)
+    double2 *T64;                 // fp64 block for pass 1 of the two-pass QR, allocated when first needed
     void *Q, *Q2, *P, *P2, *AP;   // inner-precision native blocks
     double2 *C, *Cprev, *negbeta, *W, *Sinv, *Sdag;
     double *bnorm2, *colred;
@@ -28,7 +29,7 @@ struct Workspace {
 static void free_ws(Workspace *w)
 {
     if (!w) return;
-    cudaFree(w->Bn); cudaFree(w->Xn); cudaFree(w->Y);
+    cudaFree(w->Bn); cudaFree(w->Xn); cudaFree(w->Y); cudaFree(w->T64);
     if (w->prec != BKR_F64) cudaFree(w->R64);
     cudaFree(w->Q); cudaFree(w->Q2); cudaFree(w->P); cudaFree(w->P2); cudaFree(w->AP);
     cudaFree(w->C); cudaFree(w->bnorm2); cudaFree(w->flags); cudaFree(w->cgs);
@@ -207,6 +208,9 @@ static SmallArgs small_args(Workspace *w, int mode, int num_partials, double tol
     a.tol = tol; a.delta = delta;
     a.flags = w->flags;
     a.mixed = mixed ? 1 : 0;
+    // Gram matrices of fp32 blocks (l.9, l.11 of the mixed solver) carry ~1e-7 relative rounding noise: a rank-deficient
+    // block would pass the fp64 pivot test with a noise pivot (U15)
+    if (mixed && (mode == SMALL_BETA || mode == SMALL_QR)) a.pivot_tol = 4e-6;
     return a;
 }
 
@@ -240,6 +244,31 @@ static int block_residual_qr(bkr_ctx *ctx, Workspace *w, double mass, const doub
     // Q = R C^-1 (Alg. 2 l.4), stored in the inner precision
     BKR_TRY(blk_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->R64, w->Q, nullptr, 1)); // C^-1 upper triangular
     if (fuse_qpx(ctx, N)) { // the next iteration's fused update multiplies Q by Sinv: this Q is already orthonormal
+        set_identity_kernel<<<1, 256, 0, ctx->stream>>>(N, w->Sinv);
+        BKR_TRY(bkr_check_launch(ctx));
+    }
+    return BKR_OK;
+}
+
+// Two-pass QR of the residual block left in w->R64 by block_residual_qr, whose Cholesky factorisation broke down on a
+// finite Gram matrix (nearly dependent right-hand sides): shifted Cholesky QR, then a second pass (refs [43, 44] of
+// PAPER.md:184-186; the oracle's orc_thin_qr2).  Leaves Q, C, S = 1 like SMALL_INIT; P is zeroed by the
+// caller.  flags->breakdown stays set if pass 2 finds no full rank.
+static int robust_init_qr(bkr_ctx *ctx, Workspace *w, double tol, double delta, bool mixed)
+{
+    const int N = w->N;
+    int np = 0;
+    if (!w->T64) BKR_CUDA(ctx, cudaMalloc((void **)&w->T64, w->bytes64));
+    BKR_CUDA(ctx, cudaMemsetAsync(w->flags, 0, sizeof(SolverFlags), ctx->stream));
+    BKR_CUDA(ctx, cudaMemsetAsync(&w->flags->xidle, 1, sizeof(int), ctx->stream));
+    const int *gate = &w->flags->done;
+    BKR_TRY(blk_gram(ctx, N, BKR_F64, w->R64, w->R64, &np, nullptr));
+    BKR_TRY(launch_small(ctx, small_args(w, SMALL_RQ1, np, tol, delta, mixed, ctx)));
+    BKR_TRY(blk_update(ctx, N, BKR_F64, BKR_F64, w->Sinv, nullptr, w->R64, w->T64, gate, 1)); // Q1 = R R1^-1
+    BKR_TRY(blk_gram(ctx, N, BKR_F64, w->T64, w->T64, &np, gate));
+    BKR_TRY(launch_small(ctx, small_args(w, SMALL_RQ2, np, tol, delta, mixed, ctx)));
+    BKR_TRY(blk_update(ctx, N, w->prec, BKR_F64, w->Sinv, nullptr, w->T64, w->Q, gate, 1)); // Q = Q1 R2^-1
+    if (fuse_qpx(ctx, N)) {
         set_identity_kernel<<<1, 256, 0, ctx->stream>>>(N, w->Sinv);
         BKR_TRY(bkr_check_launch(ctx));
     }
@@ -340,15 +369,21 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
     BKR_CUDA(ctx, cudaEventRecord(w->ev0, ctx->stream));
     BKR_TRY(launch_col_reduce(ctx, N, BKR_F64, 0, w->Bn, nullptr, w->bnorm2, nullptr));
 
-    int rc = BKR_OK, iters = 0, nupd = 0, restarts = 0;
+    int rc = BKR_OK, iters = 0, nupd = 0, restarts = 0, nreorth = 0, last_restart_iters = -1;
     double true_max = 0.0, iter_max = 0.0;
     const int check_every = mixed ? 1 : 8;
     for (;;) {
         BKR_TRY(reset_flags(ctx, w));
         // l.3-l.6: R = B - M X ; Q C = R ; S = 1 ; P = 0
         BKR_TRY(block_residual_qr(ctx, w, mass, mixed ? w->Y : w->Xn, SMALL_INIT, tol, delta, mixed, nullptr));
-        BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
         BKR_TRY(read_flags(ctx, w));
+        if (w->h_flags->breakdown && w->h_flags->illcond) {
+            // the residual block is (nearly) rank deficient: one Cholesky-QR pass cannot orthonormalise it, two can
+            BKR_TRY(robust_init_qr(ctx, w, tol, delta, mixed));
+            BKR_TRY(read_flags(ctx, w));
+            nreorth++;
+        }
+        BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
         int base = iters;
         while (!w->h_flags->done && iters < maxiter) {
             int batch = check_every < maxiter - iters ? check_every : maxiter - iters;
@@ -372,8 +407,18 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
             BKR_CUDA(ctx, cudaMemsetAsync(w->Xn, 0, w->bytes64, ctx->stream));
         }
         BKR_TRY(true_residuals(ctx, w, mass, mixed ? w->Y : w->Xn, true_relres, &true_max));
-        if (w->h_flags->breakdown) { rc = BKR_EBREAKDOWN; break; }
         if (true_max <= tol) { rc = BKR_OK; break; }
+        if (w->h_flags->breakdown) {
+            // a finite Gram matrix that failed the pivot test inside the loop: restart from X (the restart's QR takes the
+            // two-pass route if it has to); anything else, or a block that keeps failing, is a breakdown
+            if (w->h_flags->illcond && restarts < 8 && iters < maxiter && iters > last_restart_iters) {
+                last_restart_iters = iters;
+                restarts++;
+                continue;
+            }
+            rc = BKR_EBREAKDOWN;
+            break;
+        }
         if (iters >= maxiter || restarts >= 8) { rc = BKR_ENOCONV; break; }
         restarts++; // iterated residual passed but the true one missed tol (U10): re-enter from X
     }
@@ -387,6 +432,7 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
         stats->reliable_updates = nupd;
         stats->status = rc;
         stats->restarts = restarts;
+        stats->reorthonormalisations = nreorth;
         stats->seconds = ms * 1e-3;
         stats->true_relres_max = true_max;
         stats->iter_relres_max = iter_max;
@@ -487,6 +533,7 @@ int solver_cg(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, do
         stats->reliable_updates = 0;
         stats->status = rc;
         stats->restarts = 0;
+        stats->reorthonormalisations = 0;
         stats->seconds = ms * 1e-3;
         stats->true_relres_max = mx;
         stats->iter_relres_max = 0.0;

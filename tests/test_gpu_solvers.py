@@ -266,3 +266,28 @@ def test_duplicate_rhs_reports_breakdown_mixed(cfg1):
     B2[3] = B2[0]
     _, _, st = ctx.solve_block(0.1, torch.from_numpy(B2).cuda(), tol=TOL, inner_prec=binding.F32, delta=0.1)
     assert st["status"] == binding.EBREAKDOWN
+
+
+@pytest.mark.parametrize("inner", ["f64", "f32"])
+def test_nearly_dependent_rhs_two_pass_qr(cfg1, inner):
+    """SURVEY.md NEXT-2 (refs [43, 44]): two sources equal to 1e-7 make the Gram matrix of the initial
+    residual lose 14 digits; one Cholesky-QR pass breaks down (round 1 returned BKR_EBREAKDOWN), the two-pass QR
+    orthonormalises the block and the solve converges to what the oracle's two-pass solver and the dense solve give."""
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, B, ctx = cfg1
+    Bd = B.copy()
+    Bd[3] = Bd[1] + 1e-7 * Bd[3]
+    kw = dict(inner_prec=binding.F32, delta=0.1) if inner == "f32" else {}
+    X, rr, st = ctx.solve_block(0.1, torch.from_numpy(Bd).cuda(), tol=1e-11, **kw)
+    assert st["status"] == 0 and st["reorthonormalisations"] >= 1, st
+    Xh = X.cpu().numpy()
+    assert oracle.true_relres(dims, fat, lng, 0.1, Bd, Xh).max() <= TOL
+    ro = oracle.block_cg(dims, fat, lng, 0.1, Bd, tol=1e-11, reorth=True)
+    assert ro["status"] == 0
+    assert _soldiff(Xh, ro["X"]) <= 1e-8
+    _, _, M = H.dense_blocks(dims, fat, lng, 0.1)
+    Xs = np.linalg.solve(M, Bd.reshape(4, -1).T).T.reshape(Bd.shape)
+    assert _soldiff(Xh, Xs) <= 1e-8
+    # a well conditioned block never takes the second pass
+    _, _, st0 = ctx.solve_block(0.1, torch.from_numpy(B).cuda(), tol=TOL, **kw)
+    assert st0["status"] == 0 and st0["reorthonormalisations"] == 0
