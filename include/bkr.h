@@ -43,7 +43,7 @@
 extern "C" {
 #endif
 
-#define BKR_MAX_N 32
+#define BKR_MAX_N 64 /* blocks of more than 32 rhs must have an even N (they are worked on as two panels of N / 2) */
 
 typedef struct bkr_ctx bkr_ctx; /* opaque: device copies of the links, workspaces, stream */
 

@@ -5,7 +5,9 @@
 #include <stdlib.h>
 #include <string.h>
 
-static bool valid_n(int N) { return N >= 1 && N <= BKR_MAX_N; }
+static bool valid_n(int N) { return N >= 1 && N <= BKR_MAX_N && (N <= 32 || N % 2 == 0); }
+// fused-kernel entry points keep the 32-rhs limit of their kernels
+static bool valid_n32(int N) { return N >= 1 && N <= 32; }
 static bool valid_prec(int p) { return p == BKR_F64 || p == BKR_F32; }
 
 extern "C" {
@@ -32,7 +34,7 @@ int bkr_create(bkr_ctx **out, const int dims[4], int device, void *cuda_stream)
     ctx->dslash_variant = -1;
     ctx->dslash_force = -1;
     ctx->stream = (cudaStream_t)cuda_stream;
-    if (cudaMalloc((void **)&ctx->small, (size_t)4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)) != cudaSuccess) {
+    if (cudaMalloc((void **)&ctx->small, (size_t)5 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)) != cudaSuccess) {
         free(ctx);
         return BKR_ENOMEM;
     }
@@ -56,6 +58,7 @@ int bkr_destroy(bkr_ctx *ctx)
     cudaFree(ctx->tmp_odd[1]);
     cudaFree(ctx->partials);
     cudaFree(ctx->small);
+    cudaFree(ctx->panel);
     cudaFree(ctx->stage[0]);
     cudaFree(ctx->stage[1]);
     free(ctx);
@@ -130,6 +133,7 @@ int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int he
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !X || !Y || !K) return BKR_EINVAL;
     BKR_ENTER(ctx);
     int np = 0;
+    if (N > 32) return launch_gram_panels(ctx, N, prec, X, Y, hermitian ? 1 : 0, (double2 *)K, nullptr);
     BKR_TRY(launch_gram_partials(ctx, N, prec, X, Y, hermitian ? 1 : 0, &np, nullptr));
     return launch_gram_finish(ctx, N, np, hermitian ? 1 : 0, (double2 *)K);
 }
@@ -150,7 +154,7 @@ int bkr_block_update(bkr_ctx *ctx, int N, int precZ, int precW, int tri, const v
 
 int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y, void *K)
 {
-    if (!ctx || !valid_n(N) || !valid_prec(prec) || !a || !X || !Y || !K || X == Y) return BKR_EINVAL;
+    if (!ctx || !valid_n32(N) || !valid_prec(prec) || !a || !X || !Y || !K || X == Y) return BKR_EINVAL;
     BKR_ENTER(ctx);
     int np = 0;
     BKR_TRY(launch_update_gram(ctx, N, prec, (const double2 *)a, Y, X, Y, &np, nullptr));
@@ -160,7 +164,7 @@ int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void
 int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const void *Sdag, const void *Wm, void *Q,
                          const void *P, void *Pn, void *X, int do_qp, int do_x)
 {
-    if (!ctx || !valid_n(N) || !valid_prec(prec) || !Sinv || !Sdag || !Wm || !Q || !P || !Pn || !X || P == Pn) return BKR_EINVAL;
+    if (!ctx || !valid_n32(N) || !valid_prec(prec) || !Sinv || !Sdag || !Wm || !Q || !P || !Pn || !X || P == Pn) return BKR_EINVAL;
     BKR_ENTER(ctx);
     if (!ctx->api_flags) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->api_flags, sizeof(SolverFlags)));
     SolverFlags f;
@@ -177,7 +181,7 @@ int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const 
 
 int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, int *status)
 {
-    if (!ctx || !valid_n(N) || !H || !R) return BKR_EINVAL;
+    if (!ctx || N < 1 || N > BKR_MAX_N || !H || !R) return BKR_EINVAL;
     BKR_ENTER(ctx);
     SmallArgs a;
     memset(&a, 0, sizeof(a));
@@ -192,7 +196,7 @@ int bkr_cholesky_upper(bkr_ctx *ctx, int N, const void *H, void *R, void *Rinv, 
 
 int bkr_hpd_inverse(bkr_ctx *ctx, int N, const void *G, void *Ginv, int *status)
 {
-    if (!ctx || !valid_n(N) || !G || !Ginv) return BKR_EINVAL;
+    if (!ctx || N < 1 || N > BKR_MAX_N || !G || !Ginv) return BKR_EINVAL;
     BKR_ENTER(ctx);
     SmallArgs a;
     memset(&a, 0, sizeof(a));

@@ -15,8 +15,9 @@ int ensure_partials(bkr_ctx *ctx, size_t bytes)
 
 // ------------------------------------------------------------------------------------------ Gram, stage 2
 __global__ void gram_finish_kernel(int N, int num_partials, int hermitian, const double2 *__restrict__ partials,
-                                   double2 *__restrict__ K)
+                                   double2 *__restrict__ K, int ldk, const int *done)
 {
+    if (done && *done) return;
     int o = blockIdx.x * blockDim.x + threadIdx.x;
     if (o >= N * N) return;
     int i = o / N, j = o % N;
@@ -30,13 +31,48 @@ __global__ void gram_finish_kernel(int N, int num_partials, int hermitian, const
     }
     if (lower) s.y = -s.y;
     if (hermitian && i == j) s.y = 0.0;
-    K[o] = s;
+    K[i * ldk + j] = s;
 }
 
-int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K)
+int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K, int ldk)
 {
-    gram_finish_kernel<<<(N * N + 127) / 128, 128, 0, ctx->stream>>>(N, num_partials, hermitian, ctx->partials, K);
+    gram_finish_kernel<<<(N * N + 127) / 128, 128, 0, ctx->stream>>>(N, num_partials, hermitian, ctx->partials, K, ldk ? ldk : N,
+                                                                     nullptr);
     return bkr_check_launch(ctx);
+}
+
+// lower triangle of an N x N matrix from its upper one: K_ij = conj(K_ji), i > j
+__global__ void mirror_lower_kernel(int N, double2 *K, const int *done)
+{
+    if (done && *done) return;
+    const int o = blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= N * N) return;
+    const int i = o / N, j = o % N;
+    if (i > j) {
+        const double2 v = K[j * N + i];
+        K[o] = make_double2(v.x, -v.y);
+    }
+}
+
+int launch_gram_panels(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, double2 *K, const int *done)
+{
+    const int p = N / 2;
+    const size_t col = (size_t)3 * ctx->g.Vh * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
+    for (int I = 0; I < 2; I++)
+        for (int J = 0; J < 2; J++) {
+            if (hermitian && I > J) continue;
+            int np = 0;
+            const char *xi = (const char *)X + (size_t)I * p * col, *yj = (const char *)Y + (size_t)J * p * col;
+            BKR_TRY(launch_gram_partials(ctx, p, prec, xi, yj, (hermitian && I == J) ? 1 : 0, &np, done));
+            gram_finish_kernel<<<(p * p + 127) / 128, 128, 0, ctx->stream>>>(p, np, (hermitian && I == J) ? 1 : 0, ctx->partials,
+                                                                             K + (size_t)I * p * N + (size_t)J * p, N, done);
+            BKR_TRY(bkr_check_launch(ctx));
+        }
+    if (hermitian) {
+        mirror_lower_kernel<<<(N * N + 127) / 128, 128, 0, ctx->stream>>>(N, K, done);
+        BKR_TRY(bkr_check_launch(ctx));
+    }
+    return BKR_OK;
 }
 
 // ------------------------------------------------------------------------------------------ per-column kernels
@@ -111,7 +147,7 @@ int launch_col_reduce(bkr_ctx *ctx, int N, int prec, int mode, const void *X, co
     else
         col_reduce_kernel<float><<<grid, COL_THREADS, 0, ctx->stream>>>(L, mode, (const float2 *)X, (const float2 *)Y, part, done);
     BKR_TRY(bkr_check_launch(ctx));
-    col_finish_kernel<<<1, 32, 0, ctx->stream>>>(N, (int)gx, part, out, done);
+    col_finish_kernel<<<1, BKR_MAX_N, 0, ctx->stream>>>(N, (int)gx, part, out, done);
     return bkr_check_launch(ctx);
 }
 

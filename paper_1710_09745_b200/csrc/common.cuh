@@ -80,6 +80,7 @@ struct bkr_ctx {
     size_t partials_bytes;
     // small-matrix scratch for the API-level gram / cholesky calls
     double2 *small;
+    double2 *panel; // dense (N/2) x (N/2) copies of coefficient sub-matrices for the panel launches of blocks > 32 rhs
     // solver workspace (allocated on first solve for a given N / precision, reused)
     struct Workspace *ws;
     // device staging blocks of the host-buffer entry points (kept between calls)
@@ -146,8 +147,12 @@ int launch_dslash_row(bkr_ctx *ctx, int out_parity, int N, int prec, const void 
 // stage 1 of K = X^dag Y: per-CTA partial sums into ctx->partials; returns the number of partials.
 int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian,
                          int *num_partials, const int *done);
-// stage 2 alone (API path): K = fixed-order sum of the partials, mirrored if hermitian.
-int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K);
+// stage 2 alone (API path): K = fixed-order sum of the partials, mirrored if hermitian.  ldk: row stride of K (0 = N).
+int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K, int ldk = 0);
+// Blocks of 34..64 rhs (N even): the whole Gram matrix K (N x N, row stride N) from the panels X_I^dag Y_J of N / 2 columns
+// each -- three launches if hermitian (the lower triangle mirrored), else four; every block is read twice (PAPER.md:262-270:
+// the paper's recursive tiling, one level, on the host).
+int launch_gram_panels(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, double2 *K, const int *done);
 // Z = C + W a   (C may be NULL = 0; Z may alias C; Z must not alias W).  a: N x N complex fp64 (device).
 // precZ is the precision of Z and C, precW of W; arithmetic in precZ.
 // tri: 0 = general a, 1 = a upper triangular, 2 = a lower triangular (entries on the other side are not read).
@@ -192,6 +197,7 @@ struct SmallArgs {
     int *status;             // API path
     int mixed;
     double pivot_tol;        // breakdown when a pivot d <= pivot_tol * h_jj (0: the mode's default)
+    double2 *scratch;        // N x N in global memory (set by launch_small): the fourth work matrix when N > 56
 };
 enum { SMALL_CHOL = 0, SMALL_HPDINV = 1, SMALL_BETA = 2, SMALL_QR = 3, SMALL_INIT = 4, SMALL_RELUPD = 5, SMALL_RQ1 = 6, SMALL_RQ2 = 7 };
 int launch_small(bkr_ctx *ctx, const SmallArgs &args);

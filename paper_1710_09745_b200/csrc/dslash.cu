@@ -352,9 +352,10 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
     // read once per chunk); likewise 11-13 rhs as 8 + rest (window kernel + plain kernel) and fp32 blocks of 17-28 rhs as
     // 16 + rest.  A chunk is a contiguous view of the native block [rhs][colour][site].
     int chunk = 0;
-    if ((ctx->dslash_force < 0 || ctx->dslash_force == 1) && ctx->tune[BKR_TUNE_DSLASH_CHUNK] != 1) {
+    if (N > 32 || ((ctx->dslash_force < 0 || ctx->dslash_force == 1) && ctx->tune[BKR_TUNE_DSLASH_CHUNK] != 1)) {
         if (prec == BKR_F64 && N > 16) chunk = 16;
         else if (prec == BKR_F64 && N >= 11 && N <= 13) chunk = 8; // 14 = window cluster of 2 (1.29 ms) beats 8 + 6 (1.32 ms)
+        else if (prec == BKR_F32 && N > 32) chunk = 32; // 33..64 fp32 rhs: 32 (a window cluster of 2) + rest
         else if (prec == BKR_F32 && N > 16 && N <= 28) chunk = 16;
     }
     if (chunk) {

@@ -284,9 +284,40 @@ static int launch_update_t(bkr_ctx *ctx, int N, const double2 *a, const void *C,
 #undef UPD_GO
 }
 
+// dense p x p copy of the sub-matrix a[i0 .. i0 + p)[j0 .. j0 + p) of an N x N coefficient matrix
+__global__ void submatrix_kernel(int N, int p, int i0, int j0, const double2 *__restrict__ a, double2 *__restrict__ out, const int *done)
+{
+    if (done && *done) return;
+    const int o = blockIdx.x * blockDim.x + threadIdx.x;
+    if (o < p * p) out[o] = a[(size_t)(i0 + o / p) * N + j0 + o % p];
+}
+
 int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *a, const void *C, const void *W, void *Z,
                         const int *done, int tri)
 {
+    if (N > 32) {
+        // Blocks of 34..64 rhs (N even) as two panels of p = N / 2 columns: Z_J = C_J + W_0 a_0J + W_1 a_1J, one launch per
+        // non-zero p x p block of the coefficient matrix (one level of the paper's recursive tiling; a
+        // triangular a leaves three).  A panel is a contiguous view of the native block [rhs][colour][site].
+        const int p = N / 2;
+        const size_t L3 = (size_t)3 * ctx->g.Vh;
+        const size_t cz = L3 * (precZ == BKR_F64 ? sizeof(double2) : sizeof(float2)), cw = L3 * (precW == BKR_F64 ? sizeof(double2) : sizeof(float2));
+        if (!ctx->panel) BKR_CUDA(ctx, cudaMalloc((void **)&ctx->panel, (size_t)4 * 32 * 32 * sizeof(double2)));
+        for (int J = 0; J < 2; J++) {
+            bool first = true;
+            for (int I = 0; I < 2; I++) {
+                if ((tri == 1 && I > J) || (tri == 2 && I < J)) continue;
+                double2 *sub = ctx->panel + (size_t)(2 * I + J) * 32 * 32;
+                submatrix_kernel<<<(p * p + 127) / 128, 128, 0, ctx->stream>>>(N, p, I * p, J * p, a, sub, done);
+                BKR_TRY(bkr_check_launch(ctx));
+                char *zj = (char *)Z + (size_t)J * p * cz;
+                const char *cj = first ? (C ? (const char *)C + (size_t)J * p * cz : nullptr) : (const char *)zj;
+                BKR_TRY(launch_block_update(ctx, p, precZ, precW, sub, cj, (const char *)W + (size_t)I * p * cw, zj, done, I == J ? tri : 0));
+                first = false;
+            }
+        }
+        return BKR_OK;
+    }
     if (precZ == BKR_F64 && precW == BKR_F64) return launch_update_t<double, double>(ctx, N, a, C, W, Z, done, tri);
     if (precZ == BKR_F64 && precW == BKR_F32) return launch_update_t<double, float>(ctx, N, a, C, W, Z, done, tri);
     if (precZ == BKR_F32 && precW == BKR_F32) return launch_update_t<float, float>(ctx, N, a, C, W, Z, done, tri);

@@ -18,6 +18,8 @@
 //                 C = R2 R1; Sinv = R2^-1; then as SMALL_INIT
 #include "common.cuh"
 
+#define SMALL_SMEM4_MAX_N 56 /* 4 x 56^2 x 16 = 196 KB of shared memory; 3 x 64^2 x 16 = 192 KB */
+
 __device__ __forceinline__ double2 cmul(double2 a, double2 b)
 {
     return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
@@ -34,34 +36,36 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 b) // conj(a) * b
 // digits against the diagonal entry it started from (d <= 1e-13 h_jj: the column is linearly dependent on the
 // previous ones to working precision, and only rounding noise decides the sign of the pivot).
 // rel_tol / abs_tol: a pivot must exceed rel_tol * h_jj and abs_tol.  *finite_out: no NaN / Inf was met.
-__device__ bool warp_cholesky_upper(int N, double2 *A, int lane, double rel_tol, double abs_tol, bool *finite_out)
+__device__ bool warp_cholesky_upper(int N, double2 *A, int lane, double rel_tol, double abs_tol, bool *finite_out, double *h0)
 {
-    const double h0 = lane < N ? A[lane * N + lane].x : 0.0;
+    // one warp; a lane owns the columns lane and lane + 32 (N <= 64); h0[j] = the diagonal entry column j started from
+    for (int c = lane; c < N; c += 32) h0[c] = A[c * N + c].x;
+    __syncwarp();
     *finite_out = true;
     for (int j = 0; j < N; j++) {
-        double d = A[j * N + j].x;
-        double hjj = __shfl_sync(0xffffffffu, h0, j);
+        const double d = A[j * N + j].x, hjj = h0[j];
         if (!isfinite(d) || !isfinite(hjj)) {
             *finite_out = false;
             return false;
         }
         if (!(d > rel_tol * hjj) || !(d > abs_tol)) return false; // uniform across the warp
-        double rjj = sqrt(d);
+        const double rjj = sqrt(d);
         __syncwarp();
-        if (lane < N) {
-            if (lane == j) A[j * N + j] = make_double2(rjj, 0.0);
-            else if (lane > j) {
-                double2 v = A[j * N + lane];
-                A[j * N + lane] = make_double2(v.x / rjj, v.y / rjj);
-            } else A[j * N + lane] = make_double2(0.0, 0.0);
+        for (int c = lane; c < N; c += 32) {
+            if (c == j) A[j * N + j] = make_double2(rjj, 0.0);
+            else if (c > j) {
+                double2 v = A[j * N + c];
+                A[j * N + c] = make_double2(v.x / rjj, v.y / rjj);
+            } else A[j * N + c] = make_double2(0.0, 0.0);
         }
         __syncwarp();
-        if (lane > j && lane < N) {
-            double2 rjc = A[j * N + lane];
-            for (int i = j + 1; i <= lane; i++) {
+        for (int c = lane; c < N; c += 32) {
+            if (c <= j) continue;
+            const double2 rjc = A[j * N + c];
+            for (int i = j + 1; i <= c; i++) {
                 double2 t = cmulc(A[j * N + i], rjc);
-                double2 v = A[i * N + lane];
-                A[i * N + lane] = make_double2(v.x - t.x, v.y - t.y);
+                double2 v = A[i * N + c];
+                A[i * N + c] = make_double2(v.x - t.x, v.y - t.y);
             }
         }
         __syncwarp();
@@ -69,11 +73,10 @@ __device__ bool warp_cholesky_upper(int N, double2 *A, int lane, double rel_tol,
     return true;
 }
 
-// Ri = R^-1 for upper-triangular R with real diagonal; lane = column of Ri (back substitution).
+// Ri = R^-1 for upper-triangular R with real diagonal; a lane owns the columns lane, lane + 32 of Ri (back substitution).
 __device__ void warp_upper_inverse(int N, const double2 *R, double2 *Ri, int lane)
 {
-    if (lane < N) {
-        int c = lane;
+    for (int c = lane; c < N; c += 32) {
         for (int i = N - 1; i > c; i--) Ri[i * N + c] = make_double2(0.0, 0.0);
         Ri[c * N + c] = make_double2(1.0 / R[c * N + c].x, 0.0);
         for (int i = c - 1; i >= 0; i--) {
@@ -153,9 +156,10 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
 {
     extern __shared__ double2 sm[];
     const int N = p.N, NN = N * N;
-    double2 *A = sm, *B = sm + NN, *Cm = sm + 2 * NN, *Dm = sm + 3 * NN;
+    // four N x N matrices; above N = 56 the fourth (a read-mostly copy) lives in global memory: 4 x 64^2 x 16 bytes do not fit
+    double2 *A = sm, *B = sm + NN, *Cm = sm + 2 * NN, *Dm = N > SMALL_SMEM4_MAX_N ? p.scratch : sm + 3 * NN;
     __shared__ int ok_s, finite_s;
-    __shared__ double scratch[BKR_MAX_N];
+    __shared__ double scratch[BKR_MAX_N], h0s[BKR_MAX_N];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     SolverFlags *fl = p.flags;
     if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) {
@@ -181,7 +185,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
         // pivot below 1e-8 is the image of rounding noise (no full rank).
         const double rel = p.pivot_tol > 0.0 ? p.pivot_tol : 1e-13;
         bool fin = true;
-        bool ok = warp_cholesky_upper(N, A, lane, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin); // A = R
+        bool ok = warp_cholesky_upper(N, A, lane, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin, h0s); // A = R
         if (ok) warp_upper_inverse(N, A, B, lane); // B = R^-1
         if (lane == 0) {
             ok_s = ok ? 1 : 0;
@@ -363,13 +367,16 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
     }
 }
 
-int launch_small(bkr_ctx *ctx, const SmallArgs &args)
+int launch_small(bkr_ctx *ctx, const SmallArgs &args_in)
 {
-    size_t smem = (size_t)4 * args.N * args.N * sizeof(double2);
+    SmallArgs args = args_in;
+    args.scratch = ctx->small + (size_t)4 * BKR_MAX_N * BKR_MAX_N;
+    const size_t nmat = args.N > SMALL_SMEM4_MAX_N ? 3 : 4;
+    size_t smem = nmat * args.N * args.N * sizeof(double2);
     static int attr_dev = -1; // the opt-in is per device
     if (attr_dev != ctx->device) {
         cudaFuncSetAttribute(small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(4 * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
+                             (int)(4 * SMALL_SMEM4_MAX_N * SMALL_SMEM4_MAX_N * sizeof(double2)));
         attr_dev = ctx->device;
     }
     small_kernel<<<1, 256, smem, ctx->stream>>>(args);
@@ -411,6 +418,6 @@ __global__ void cg_scalar_kernel(int N, int step, double tol, CgScalars *s, Solv
 
 int launch_cg_scalar(bkr_ctx *ctx, int N, int step, double tol, CgScalars *s, SolverFlags *flags)
 {
-    cg_scalar_kernel<<<1, 32, 0, ctx->stream>>>(N, step, tol, s, flags);
+    cg_scalar_kernel<<<1, BKR_MAX_N, 0, ctx->stream>>>(N, step, tol, s, flags);
     return bkr_check_launch(ctx);
 }

@@ -173,7 +173,13 @@ static int blk_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2 *
 // stage 1 of a Hermitian Gram matrix K = X^dag Y; *np = number of partials, 0 when K itself is already in ctx->small
 static int blk_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int *np, const int *done)
 {
-    if (!(ctx->ablation & BKR_ABL_VECTOR_BLAS)) return launch_gram_partials(ctx, N, prec, X, Y, 1, np, done);
+    if (!(ctx->ablation & BKR_ABL_VECTOR_BLAS)) {
+        if (N > 32) { // two panels: the whole matrix lands in ctx->small, the small-matrix kernel reads it from there
+            *np = 0;
+            return launch_gram_panels(ctx, N, prec, X, Y, 1, ctx->small, done);
+        }
+        return launch_gram_partials(ctx, N, prec, X, Y, 1, np, done);
+    }
     const size_t sv = (size_t)3 * ctx->g.Vh * (prec == BKR_F64 ? sizeof(double2) : sizeof(float2));
     for (int i = 0; i < N; i++)
         for (int j = i; j < N; j++) {
