@@ -157,6 +157,17 @@ int bkr_solve_block(bkr_ctx *ctx, double mass, int N, const void *B, void *X, do
 int bkr_solve_cg(bkr_ctx *ctx, double mass, int N, const void *B, void *X, double tol, int maxiter,
                  int batched, int *iters, double *true_relres, bkr_stats *stats);
 
+/* Workload driver of the paper's model test (192 rhs solved in blocks of N = 8 .. 64, sloppy
+ * sweep to 5e-6 and fine sweep to 2e-9 as in the Truncated Solver Method): nrhs right-hand sides, nrhs a multiple of
+ * N, solved block by block with bkr_solve_block.  Sweep 0 solves every block to tol_sloppy from the X given on entry
+ * (skipped when tol_sloppy <= 0); sweep 1 solves it to tol_fine starting from the result of sweep 0.
+ * B, X: DEVICE, canonical fp64, (nrhs, Vh, 3); block b is rhs [b N, (b + 1) N).
+ * true_relres: HOST array of nrhs doubles, after the last sweep (may be NULL).
+ * stats: HOST array of 2 * (nrhs / N) entries, stats[2 b + sweep] (may be NULL; a skipped sweep is zeroed).
+ * Returns the first non-zero status of a block solve (later blocks are still solved), else BKR_OK. */
+int bkr_solve_many(bkr_ctx *ctx, double mass, int nrhs, int N, const void *B, void *X, double tol_sloppy, double tol_fine,
+                   int maxiter, int inner_prec, double delta, double *true_relres, bkr_stats *stats);
+
 /* End-to-end variants: B and X are HOST arrays (canonical fp64); the host->device copy of B and X0 and
  * the device->host copy of X run inside the call. */
 int bkr_solve_block_host(bkr_ctx *ctx, double mass, int N, const void *B_host, void *X_host, double tol,

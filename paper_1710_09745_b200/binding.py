@@ -23,7 +23,7 @@ SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash", "bkr_dslash_xpay",
     "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_update", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
-    "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench", "bkr_solver_state",
+    "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench", "bkr_solver_state", "bkr_solve_many",
 )
 
 
@@ -76,6 +76,7 @@ def lib():
             "bkr_hpd_inverse": (ci, [vp, ci, vp, vp, vp]),
             "bkr_solve_block": (ci, [vp, cd, ci, vp, vp, cd, ci, ci, cd, vp, ctypes.POINTER(Stats)]),
             "bkr_solve_cg": (ci, [vp, cd, ci, vp, vp, cd, ci, ci, vp, vp, ctypes.POINTER(Stats)]),
+            "bkr_solve_many": (ci, [vp, cd, ci, ci, vp, vp, cd, cd, ci, ci, cd, vp, ctypes.POINTER(Stats)]),
             "bkr_solve_block_host": (ci, [vp, cd, ci, vp, vp, cd, ci, ci, cd, vp, ctypes.POINTER(Stats)]),
             "bkr_solve_cg_host": (ci, [vp, cd, ci, vp, vp, cd, ci, ci, vp, vp, ctypes.POINTER(Stats)]),
             "bkr_bench_iterations": (ci, [vp, cd, ci, ci, vp, ci, ctypes.POINTER(ctypes.c_longlong)]),
@@ -267,6 +268,19 @@ class Context:
                                    int(inner_prec), float(delta), rr, ctypes.byref(st))
         self._check(rc, "bkr_solve_block", allow=(EBREAKDOWN, ENOCONV))
         return X, list(rr), st.as_dict()
+
+    def solve_many(self, mass, B, N, tol_sloppy=5e-6, tol_fine=2e-9, X0=None, maxiter=10000, inner_prec=F64, delta=0.1):
+        """nrhs = B.shape[0] right-hand sides in blocks of N, sloppy + fine sweep (bkr_solve_many).  Returns X, the true
+        relative residuals after the last sweep and stats[block][sweep] as dicts."""
+        nrhs = int(B.shape[0])
+        X = torch.zeros_like(B) if X0 is None else X0.clone()
+        rr = (ctypes.c_double * nrhs)()
+        nb = nrhs // int(N)
+        st = (Stats * (2 * nb))()
+        rc = lib().bkr_solve_many(self._h, float(mass), nrhs, int(N), _dev_ptr(B, "B"), _dev_ptr(X, "X"), float(tol_sloppy),
+                                  float(tol_fine), int(maxiter), int(inner_prec), float(delta), rr, st)
+        self._check(rc, "bkr_solve_many", allow=(EBREAKDOWN, ENOCONV))
+        return X, list(rr), [[st[2 * b + s].as_dict() for s in range(2)] for b in range(nb)]
 
     def solve_cg(self, mass, B, X0=None, tol=1e-10, maxiter=10000, batched=False):
         N = self._n_of(B)

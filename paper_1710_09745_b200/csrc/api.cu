@@ -226,6 +226,34 @@ int bkr_solve_block(bkr_ctx *ctx, double mass, int N, const void *B, void *X, do
     return rc;
 }
 
+int bkr_solve_many(bkr_ctx *ctx, double mass, int nrhs, int N, const void *B, void *X, double tol_sloppy, double tol_fine,
+                   int maxiter, int inner_prec, double delta, double *true_relres, bkr_stats *stats)
+{
+    if (!valid_solve(ctx, N, B, X, tol_fine, maxiter) || !valid_prec(inner_prec) || nrhs < N || nrhs % N != 0) return BKR_EINVAL;
+    BKR_ENTER(ctx);
+    if (inner_prec == BKR_F32 && !(delta > 0.0 && delta < 1.0)) return BKR_EINVAL;
+    if (!ctx->links64 || (inner_prec == BKR_F32 && !ctx->links32)) return BKR_ENOLINKS;
+    const size_t blk = (size_t)N * ctx->g.Vh * 3; // complex numbers per block
+    int first = BKR_OK;
+    for (int b = 0; b < nrhs / N; b++) {
+        const double2 *Bb = (const double2 *)B + (size_t)b * blk;
+        double2 *Xb = (double2 *)X + (size_t)b * blk;
+        for (int sweep = 0; sweep < 2; sweep++) {
+            bkr_stats *st = stats ? stats + 2 * b + sweep : nullptr;
+            if (sweep == 0 && !(tol_sloppy > 0.0)) {
+                if (st) memset(st, 0, sizeof(*st));
+                continue;
+            }
+            const int rc = solver_block(ctx, mass, N, Bb, Xb, sweep == 0 ? tol_sloppy : tol_fine, maxiter, inner_prec, delta,
+                                        true_relres ? true_relres + (size_t)b * N : nullptr, st);
+            if (st) st->status = rc;
+            if (rc != BKR_OK && first == BKR_OK) first = rc;
+            if (rc == BKR_ECUDA || rc == BKR_ENOMEM) return rc;
+        }
+    }
+    return first;
+}
+
 int bkr_solve_cg(bkr_ctx *ctx, double mass, int N, const void *B, void *X, double tol, int maxiter, int batched,
                  int *iters, double *true_relres, bkr_stats *stats)
 {

@@ -161,3 +161,30 @@ def test_block_solve_large_block_mixed(lat8):
     X, rr, st = ctx.solve_block(0.05, torch.from_numpy(B).cuda(), tol=1e-10, inner_prec=binding.F32, delta=0.1)
     assert st["status"] == 0 and st["reliable_updates"] >= 1
     assert oracle.true_relres(dims, fat, lng, 0.05, B, X.cpu().numpy()).max() <= 1e-10
+
+
+@pytest.mark.parametrize("inner", ["f64", "f32"])
+def test_solve_many_blocks_sloppy_and_fine(lat, inner):
+    """bkr_solve_many (many rhs in blocks of N, sloppy sweep then fine sweep): 24 sources in blocks of 8
+    against the oracle run block by block; the fine sweep starts from the sloppy solution, so it needs fewer iterations
+    than a fine solve from zero"""
+    from paper_1710_09745_b200 import binding
+    dims, fat, lng, ctx = lat
+    nrhs, N = 24, 8
+    B = H.np_sources(dims, nrhs, 4500)
+    kw = dict(inner_prec=binding.F32, delta=0.1) if inner == "f32" else {}
+    X, rr, st = ctx.solve_many(0.1, torch.from_numpy(B).cuda(), N, tol_sloppy=5e-6, tol_fine=2e-9, **kw)
+    Xh = X.cpu().numpy()
+    assert len(st) == 3 and all(s[0]["status"] == 0 and s[1]["status"] == 0 for s in st)
+    assert max(rr) <= 2e-9
+    for b in range(3):
+        Bb = B[b * N:(b + 1) * N]
+        assert oracle.true_relres(dims, fat, lng, 0.1, Bb, Xh[b * N:(b + 1) * N]).max() <= 2e-9
+        ro = oracle.block_cg(dims, fat, lng, 0.1, Bb, tol=2e-9)
+        assert ro["status"] == 0
+        assert np.abs(Xh[b * N:(b + 1) * N] - ro["X"]).max() <= 1e-7 * np.abs(ro["X"]).max()
+        assert st[b][0]["iters"] > 0 and 0 < st[b][1]["iters"] < ro["iters"]
+        assert st[b][0]["true_relres_max"] <= 5e-6
+    # fine sweep only
+    X2, rr2, st2 = ctx.solve_many(0.1, torch.from_numpy(B).cuda(), N, tol_sloppy=0.0, tol_fine=2e-9, **kw)
+    assert all(s[0]["iters"] == 0 and s[1]["status"] == 0 for s in st2) and max(rr2) <= 2e-9
