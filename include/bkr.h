@@ -222,7 +222,8 @@ enum {
     BKR_ABL_UNFUSED_UPDATES = 1, /* Q, P, X updates as separate kernels, X updated right after Alg. 1 l.9 (no deferral)   */
     BKR_ABL_UNFUSED_GRAM = 2,    /* Q' = Q - MP beta and its Gram matrix as two kernels                                  */
     BKR_ABL_VECTOR_BLAS = 4,     /* block updates / Gram matrices as N^2 single-vector caxpys / dot products */
-    BKR_ABL_VECTOR_DSLASH = 8    /* the stencil one rhs at a time: links re-read for every rhs         */
+    BKR_ABL_VECTOR_DSLASH = 8,   /* the stencil one rhs at a time: links re-read for every rhs         */
+    BKR_ABL_NO_GRAPH = 16        /* batches of iterations as individual launches instead of one CUDA graph               */
 };
 int bkr_set_option(bkr_ctx *ctx, int option, int value);
 

@@ -373,7 +373,7 @@ int bkr_set_option(bkr_ctx *ctx, int option, int value)
     case BKR_OPT_L2_BUDGET_MB: ctx->l2_budget_mb = value; break;
     case BKR_OPT_ROW_UNIT_TILES: ctx->row_unit_tiles = value; break;
     case BKR_OPT_ROW_VEC_POLICY: ctx->row_vec_policy = value; break;
-    case BKR_OPT_ABLATION: ctx->ablation = value & 15; break;
+    case BKR_OPT_ABLATION: ctx->ablation = value & 31; break;
     default:
         if (option < BKR_OPT_TUNE || option >= BKR_OPT_TUNE + BKR_TUNE_COUNT) return BKR_EINVAL;
         ctx->tune[option - BKR_OPT_TUNE] = value;

@@ -18,6 +18,7 @@
 //                 C = R2 R1; Sinv = R2^-1; then as SMALL_INIT
 #include "common.cuh"
 
+#define SMALL_THREADS 1024
 #define SMALL_SMEM4_MAX_N 56 /* 4 x 56^2 x 16 = 196 KB of shared memory; 3 x 64^2 x 16 = 192 KB */
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b)
@@ -30,17 +31,21 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 b) // conj(a) * b
 }
 
 // In-place upper Cholesky of the Hermitian matrix whose upper triangle is in A (row-major, shared memory).
-// On return A = R (upper triangular, real positive diagonal, zeros below).  One warp; lane = column.
+// On return A = R (upper triangular, real positive diagonal, zeros below).  Whole CTA, right-looking: per column j one
+// pivot test, the scaling of row j and the rank-1 update of the trailing triangle spread over all threads, three
+// barriers (round 1 did this in one warp, a column per lane: 57 us per call at N = 16, most of it dependent
+// shared-memory round trips).  Per element the operations and their order are those of the column version.
 //
 // Breakdown (U15): a pivot that is non-finite, non-positive, or has lost more than 13
 // digits against the diagonal entry it started from (d <= 1e-13 h_jj: the column is linearly dependent on the
 // previous ones to working precision, and only rounding noise decides the sign of the pivot).
-// rel_tol / abs_tol: a pivot must exceed rel_tol * h_jj and abs_tol.  *finite_out: no NaN / Inf was met.
-__device__ bool warp_cholesky_upper(int N, double2 *A, int lane, double rel_tol, double abs_tol, bool *finite_out, double *h0)
+// rel_tol / abs_tol: a pivot must exceed rel_tol * h_jj and abs_tol.  *finite_out: no NaN / Inf was met.  The return
+// value and *finite_out are the same in every thread (they depend on shared-memory values read after a barrier).
+__device__ bool cta_cholesky_upper(int N, double2 *A, double rel_tol, double abs_tol, bool *finite_out, double *h0)
 {
-    // one warp; a lane owns the columns lane and lane + 32 (N <= 64); h0[j] = the diagonal entry column j started from
-    for (int c = lane; c < N; c += 32) h0[c] = A[c * N + c].x;
-    __syncwarp();
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (int c = tid; c < N; c += nt) h0[c] = A[c * N + c].x;
+    __syncthreads();
     *finite_out = true;
     for (int j = 0; j < N; j++) {
         const double d = A[j * N + j].x, hjj = h0[j];
@@ -48,88 +53,113 @@ __device__ bool warp_cholesky_upper(int N, double2 *A, int lane, double rel_tol,
             *finite_out = false;
             return false;
         }
-        if (!(d > rel_tol * hjj) || !(d > abs_tol)) return false; // uniform across the warp
+        if (!(d > rel_tol * hjj) || !(d > abs_tol)) return false;
         const double rjj = sqrt(d);
-        __syncwarp();
-        for (int c = lane; c < N; c += 32) {
+        __syncthreads(); // everyone has read the pivot
+        for (int c = tid; c < N; c += nt) {
             if (c == j) A[j * N + j] = make_double2(rjj, 0.0);
             else if (c > j) {
                 double2 v = A[j * N + c];
                 A[j * N + c] = make_double2(v.x / rjj, v.y / rjj);
             } else A[j * N + c] = make_double2(0.0, 0.0);
         }
-        __syncwarp();
-        for (int c = lane; c < N; c += 32) {
-            if (c <= j) continue;
-            const double2 rjc = A[j * N + c];
-            for (int i = j + 1; i <= c; i++) {
-                double2 t = cmulc(A[j * N + i], rjc);
-                double2 v = A[i * N + c];
-                A[i * N + c] = make_double2(v.x - t.x, v.y - t.y);
-            }
+        __syncthreads();
+        const int m = N - j - 1; // trailing block: rows / columns j + 1 .. N - 1, upper triangle
+        for (int o = tid; o < m * m; o += nt) {
+            const int i = j + 1 + o / m, c = j + 1 + o % m;
+            if (c < i) continue;
+            const double2 t = cmulc(A[j * N + i], A[j * N + c]);
+            const double2 v = A[i * N + c];
+            A[i * N + c] = make_double2(v.x - t.x, v.y - t.y);
         }
-        __syncwarp();
+        __syncthreads();
     }
     return true;
 }
 
-// Ri = R^-1 for upper-triangular R with real diagonal; a lane owns the columns lane, lane + 32 of Ri (back substitution).
-__device__ void warp_upper_inverse(int N, const double2 *R, double2 *Ri, int lane)
+// Ri = R^-1 for upper-triangular R with real diagonal, whole CTA: the entries at distance d = c - i from the diagonal
+// depend only on those at smaller distances, so each distance is one parallel step (a dot product of length d per entry,
+// summed in the order of the column-wise back substitution).
+__device__ void cta_upper_inverse(int N, const double2 *R, double2 *Ri)
 {
-    for (int c = lane; c < N; c += 32) {
-        for (int i = N - 1; i > c; i--) Ri[i * N + c] = make_double2(0.0, 0.0);
-        Ri[c * N + c] = make_double2(1.0 / R[c * N + c].x, 0.0);
-        for (int i = c - 1; i >= 0; i--) {
+    const int tid = threadIdx.x, nt = blockDim.x;
+    for (int o = tid; o < N * N; o += nt) {
+        const int i = o / N, c = o % N;
+        if (i > c) Ri[o] = make_double2(0.0, 0.0);
+        else if (i == c) Ri[o] = make_double2(1.0 / R[o].x, 0.0);
+    }
+    __syncthreads();
+    for (int d = 1; d < N; d++) {
+        for (int i = tid; i + d < N; i += nt) {
+            const int c = i + d;
             double2 s = make_double2(0.0, 0.0);
             for (int k = i + 1; k <= c; k++) {
                 double2 t = cmul(R[i * N + k], Ri[k * N + c]);
                 s.x += t.x;
                 s.y += t.y;
             }
-            double d = R[i * N + i].x;
-            Ri[i * N + c] = make_double2(-s.x / d, -s.y / d);
+            const double dd = R[i * N + i].x;
+            Ri[i * N + c] = make_double2(-s.x / dd, -s.y / dd);
         }
+        __syncthreads();
     }
-    __syncwarp();
 }
 
 __device__ void load_hermitian(const SmallArgs &p, double2 *A)
 {
     const int N = p.N;
-    for (int o = threadIdx.x; o < N * N; o += blockDim.x) {
-        int i = o / N, j = o % N;
-        int src = i <= j ? o : j * N + i;
-        double2 s = make_double2(0.0, 0.0);
-        if (p.num_partials > 0) {
-            // fixed order, hence deterministic (P12): four interleaved running sums (q mod 4) combined at the end, the
-            // loads unrolled eight deep -- one serial chain of ~148 dependent L2 loads cost 54 us per call
-            double2 acc4[4];
+    if (p.num_partials > 0) {
+        // Second stage of the Gram reduction, fixed order, hence deterministic (P12): the partials q = 0, 1, 2, ... go to
+        // four running sums by q mod 4, combined as (s0 + s1) + (s2 + s3).  Four adjacent lanes hold the four sums of
+        // one matrix element (eight loads in flight each) and meet through shuffles: one serial chain of ~148 dependent
+        // L2 loads cost 54 us per call, four interleaved chains in one thread ~10 us.
+        const int g = threadIdx.x & 3, lane = threadIdx.x & 31, per = blockDim.x >> 2;
+        const size_t stride = (size_t)N * N;
+        for (int o0 = 0; o0 < N * N; o0 += per) {
+            const int o = o0 + (threadIdx.x >> 2);
+            const bool act = o < N * N;
+            const int i = act ? o / N : 0, j = act ? o % N : 0;
+            const int src = i <= j ? i * N + j : j * N + i;
+            double2 acc = make_double2(0.0, 0.0);
+            if (act) {
+                const double2 *pp = p.partials + src;
+                int q = g;
+                for (; q + 28 < p.num_partials; q += 32) {
+                    double2 v[8];
 #pragma unroll
-            for (int c = 0; c < 4; c++) acc4[c] = make_double2(0.0, 0.0);
-            const double2 *pp = p.partials + src;
-            const size_t stride = (size_t)N * N;
-            int q = 0;
-            for (; q + 8 <= p.num_partials; q += 8) {
-                double2 v[8];
+                    for (int c = 0; c < 8; c++) v[c] = pp[(size_t)(q + 4 * c) * stride];
 #pragma unroll
-                for (int c = 0; c < 8; c++) v[c] = pp[(size_t)(q + c) * stride];
-#pragma unroll
-                for (int c = 0; c < 8; c++) {
-                    acc4[c & 3].x += v[c].x;
-                    acc4[c & 3].y += v[c].y;
+                    for (int c = 0; c < 8; c++) {
+                        acc.x += v[c].x;
+                        acc.y += v[c].y;
+                    }
+                }
+                for (; q < p.num_partials; q += 4) {
+                    const double2 v = pp[(size_t)q * stride];
+                    acc.x += v.x;
+                    acc.y += v.y;
                 }
             }
-            for (; q < p.num_partials; q++) {
-                const double2 v = pp[(size_t)q * stride];
-                acc4[q & 3].x += v.x;
-                acc4[q & 3].y += v.y;
+            const int b0 = lane & ~3;
+            const double x0 = __shfl_sync(0xffffffffu, acc.x, b0), x1 = __shfl_sync(0xffffffffu, acc.x, b0 + 1),
+                         x2 = __shfl_sync(0xffffffffu, acc.x, b0 + 2), x3 = __shfl_sync(0xffffffffu, acc.x, b0 + 3);
+            const double y0 = __shfl_sync(0xffffffffu, acc.y, b0), y1 = __shfl_sync(0xffffffffu, acc.y, b0 + 1),
+                         y2 = __shfl_sync(0xffffffffu, acc.y, b0 + 2), y3 = __shfl_sync(0xffffffffu, acc.y, b0 + 3);
+            if (act && g == 0) {
+                double2 s = make_double2((x0 + x1) + (x2 + x3), (y0 + y1) + (y2 + y3));
+                if (i > j) s.y = -s.y;
+                if (i == j) s.y = 0.0;
+                A[o] = s;
             }
-            s.x = (acc4[0].x + acc4[1].x) + (acc4[2].x + acc4[3].x);
-            s.y = (acc4[0].y + acc4[1].y) + (acc4[2].y + acc4[3].y);
-        } else s = p.in[src];
-        if (i > j) s.y = -s.y;
-        if (i == j) s.y = 0.0;
-        A[o] = s;
+        }
+    } else {
+        for (int o = threadIdx.x; o < N * N; o += blockDim.x) {
+            const int i = o / N, j = o % N;
+            double2 s = p.in[i <= j ? o : j * N + i];
+            if (i > j) s.y = -s.y;
+            if (i == j) s.y = 0.0;
+            A[o] = s;
+        }
     }
     __syncthreads();
 }
@@ -152,7 +182,7 @@ __device__ double max_relres(int N, const double2 *C, const double *bnorm2, doub
     return m;
 }
 
-__global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
+__global__ void __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
 {
     extern __shared__ double2 sm[];
     const int N = p.N, NN = N * N;
@@ -160,7 +190,6 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
     double2 *A = sm, *B = sm + NN, *Cm = sm + 2 * NN, *Dm = N > SMALL_SMEM4_MAX_N ? p.scratch : sm + 3 * NN;
     __shared__ int ok_s, finite_s;
     __shared__ double scratch[BKR_MAX_N], h0s[BKR_MAX_N];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     SolverFlags *fl = p.flags;
     if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) {
         if (p.mode == SMALL_BETA && threadIdx.x == 0) { // no new W: nothing left to apply to X after this iteration
@@ -178,16 +207,16 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
         if (threadIdx.x < N) A[threadIdx.x * N + threadIdx.x].x += 1e-12 * hmax;
         __syncthreads();
     }
-    if (warp == 0) {
+    {
         // Breakdown thresholds (U15): 13 digits lost against the diagonal entry for Gram matrices of fp64 blocks;
         // fp32 blocks carry rounding noise of ~1e-7 h_jj, so a rank-deficient one would pass that test with a noise pivot:
         // the caller passes pivot_tol = 4e-6 there.  Pass 2 of the two-pass QR: columns have norm <= 1 after pass 1, a
         // pivot below 1e-8 is the image of rounding noise (no full rank).
         const double rel = p.pivot_tol > 0.0 ? p.pivot_tol : 1e-13;
         bool fin = true;
-        bool ok = warp_cholesky_upper(N, A, lane, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin, h0s); // A = R
-        if (ok) warp_upper_inverse(N, A, B, lane); // B = R^-1
-        if (lane == 0) {
+        bool ok = cta_cholesky_upper(N, A, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin, h0s); // A = R
+        if (ok) cta_upper_inverse(N, A, B); // B = R^-1
+        if (threadIdx.x == 0) {
             ok_s = ok ? 1 : 0;
             finite_s = fin ? 1 : 0;
         }
@@ -335,8 +364,7 @@ __global__ void __launch_bounds__(256) small_kernel(SmallArgs p)
         // A = C_new, B = C_new^-1.  S = C_new Cprev^-1 (Alg. 3 l.6, C_old = C before this iteration's l.12: U12)
         for (int o = threadIdx.x; o < NN; o += blockDim.x) Dm[o] = p.Cprev[o];
         __syncthreads();
-        if (warp == 0) warp_upper_inverse(N, Dm, Cm, lane); // Cm = Cprev^-1
-        __syncthreads();
+        cta_upper_inverse(N, Dm, Cm); // Cm = Cprev^-1
         for (int o = threadIdx.x; o < NN; o += blockDim.x) {
             int i = o / N, j = o % N;
             double2 s = make_double2(0.0, 0.0);
@@ -379,7 +407,7 @@ int launch_small(bkr_ctx *ctx, const SmallArgs &args_in)
                              (int)(4 * SMALL_SMEM4_MAX_N * SMALL_SMEM4_MAX_N * sizeof(double2)));
         attr_dev = ctx->device;
     }
-    small_kernel<<<1, 256, smem, ctx->stream>>>(args);
+    small_kernel<<<1, SMALL_THREADS, smem, ctx->stream>>>(args);
     return bkr_check_launch(ctx);
 }
 

@@ -378,6 +378,10 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
     int rc = BKR_OK, iters = 0, nupd = 0, restarts = 0, nreorth = 0, last_restart_iters = -1;
     double true_max = 0.0, iter_max = 0.0;
     const int check_every = mixed ? 1 : 8;
+    const bool use_graph = !mixed && !(ctx->ablation & BKR_ABL_NO_GRAPH);
+    cudaGraphExec_t gexec = nullptr;
+    bool graph_failed = false;
+    long long graph_launches = 0;
     for (;;) {
         BKR_TRY(reset_flags(ctx, w));
         // l.3-l.6: R = B - M X ; Q C = R ; S = 1 ; P = 0
@@ -391,9 +395,39 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
         }
         BKR_CUDA(ctx, cudaMemsetAsync(w->P, 0, w->bytesP, ctx->stream));
         int base = iters;
+        int eager_batches = 0;
         while (!w->h_flags->done && iters < maxiter) {
             int batch = check_every < maxiter - iters ? check_every : maxiter - iters;
-            for (int b = 0; b < batch; b++) BKR_TRY(block_iteration(ctx, w, mass, tol, delta, mixed));
+            // A full batch of the fp64 solver is one CUDA graph: every loop kernel gates itself on
+            // flags->done and an even number of iterations brings the P / Q buffer pairs back to where they started, so the
+            // same graph is launched batch after batch.  It is captured after one eager batch (tables, attributes and
+            // scratch buffers exist by then); anything the capture does not accept falls back to eager launches.
+            if (use_graph && batch == check_every && eager_batches >= 1 && !gexec && !graph_failed) {
+                const long long l0 = ctx->launches;
+                cudaGraph_t graph = nullptr;
+                int crc = BKR_OK;
+                if (cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed) == cudaSuccess) {
+                    for (int b = 0; b < batch && crc == BKR_OK; b++) crc = block_iteration(ctx, w, mass, tol, delta, mixed);
+                    const cudaError_t ce = cudaStreamEndCapture(ctx->stream, &graph);
+                    if (crc == BKR_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&gexec, graph, 0) == cudaSuccess) {
+                        graph_launches = ctx->launches - l0;
+                    } else {
+                        gexec = nullptr;
+                        graph_failed = true;
+                    }
+                    if (graph) cudaGraphDestroy(graph);
+                } else graph_failed = true;
+                cudaGetLastError();
+                ctx->launches = l0; // nothing ran during the capture
+                if (crc != BKR_OK && crc != BKR_ECUDA) return crc;
+            }
+            if (gexec && batch == check_every) {
+                BKR_CUDA(ctx, cudaGraphLaunch(gexec, ctx->stream));
+                ctx->launches += graph_launches;
+            } else {
+                for (int b = 0; b < batch; b++) BKR_TRY(block_iteration(ctx, w, mass, tol, delta, mixed));
+                eager_batches++;
+            }
             BKR_TRY(read_flags(ctx, w));
             iters = base + w->h_flags->iters;
             if (mixed && w->h_flags->want_update && !w->h_flags->done) {
@@ -428,6 +462,7 @@ int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X,
         if (iters >= maxiter || restarts >= 8) { rc = BKR_ENOCONV; break; }
         restarts++; // iterated residual passed but the true one missed tol (U10): re-enter from X
     }
+    if (gexec) cudaGraphExecDestroy(gexec);
     BKR_CUDA(ctx, cudaEventRecord(w->ev1, ctx->stream));
     BKR_TRY(launch_unpack(ctx, N, BKR_F64, mixed ? w->Y : w->Xn, X));
     BKR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
