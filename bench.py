@@ -202,6 +202,30 @@ def run_microbench(ctx, reps=5):
     return out
 
 
+# on-chip probes of csrc/probes.cu (kind, name, what the number is): cycles of one SM and work per SM -> per-cycle rates
+PROBE_KINDS = [(10, "lds128_conflict_free_B_per_clk_sm", "bytes"), (11, "lds128_broadcast8_B_per_clk_sm", "bytes"),
+               (12, "lds128_with_tma_fills_B_per_clk_sm", "bytes+aux"), (13, "lds128_with_ldg_stream_B_per_clk_sm", "bytes+aux"),
+               (14, "dfma_2_register_reads_per_clk_sm", "dfma"), (15, "dfma_3_register_reads_per_clk_sm", "dfma"),
+               (16, "dfma_with_4_lds128_per_64_per_clk_sm", "dfma"), (17, "dfma_with_8_lds128_per_64_per_clk_sm", "dfma"),
+               (18, "dry_stencil_T4_8warps_dfma_per_clk_sm", "dfma"), (19, "dry_stencil_T8_4warps_dfma_per_clk_sm", "dfma"),
+               (20, "dry_stencil_T8_8warps_dfma_per_clk_sm", "dfma"),
+               (21, "tma_9KB_issue_interval_clk_one_lane", "interval"), (22, "tma_9KB_round_trip_clk_idle_l2", "interval")]
+
+
+def run_probes(ctx):
+    """the probes behind the stencil design (profiles/r2_onchip_probes.md), as per-cycle, per-SM rates"""
+    out = {}
+    for kind, name, what in PROBE_KINDS:
+        cyc, units, aux = ctx.probe(kind)
+        if what == "interval":
+            out[name] = cyc / units
+        else:
+            out[name] = units / cyc
+            if what.endswith("+aux"):
+                out[name.replace("lds128_", "other_stream_")] = aux / cyc
+    return out
+
+
 def alu_peak_gflops(fp64):
     return ALU_PEAK[bool(fp64)]
 
@@ -643,7 +667,9 @@ def main():
         return run_sweep(args)
     if args.microbench:
         from paper_1710_09745_b200 import binding
-        print(json.dumps({"microbench": run_microbench(binding.Context((8, 8, 8, 8)), reps=10), "unit": "TFLOP/s or TB/s"}))
+        c8 = binding.Context((8, 8, 8, 8))
+        print(json.dumps({"microbench": run_microbench(c8, reps=10), "unit": "TFLOP/s or TB/s", "probes": run_probes(c8),
+                          "probes_unit": "per SM clock and SM (64 = FP64 peak, 128 B = shared-memory port) or clocks"}))
         return 0
     return run_bkr(args)
 

@@ -332,9 +332,15 @@ class Context:
 
     def microbench(self, kind, reps=5):
         """(ms per launch, flop or bytes per launch) of the on-chip microbenchmark `kind` (bkr.h)."""
-        r = (ctypes.c_double * 2)()
+        r = (ctypes.c_double * 4)()
         self._check(lib().bkr_microbench(self._h, int(kind), int(reps), r), "bkr_microbench")
         return float(r[0]), float(r[1])
+
+    def probe(self, kind):
+        """on-chip probe `kind` (10..22, csrc/probes.cu): (SM cycles, work units per SM, second work count)"""
+        r = (ctypes.c_double * 4)()
+        self._check(lib().bkr_microbench(self._h, int(kind), 1, r), "bkr_microbench")
+        return float(r[0]), float(r[1]), float(r[2])
 
     def set_option(self, option, value):
         """launch-policy knob (bkr.h BKR_OPT_*): OPT_L2_BUDGET_MB = 0, OPT_ROW_UNIT_TILES = 1; value 0 = default."""

@@ -211,6 +211,8 @@ int launch_cg_scalar(bkr_ctx *ctx, int N, int step, double tol, CgScalars *s, So
 
 // ---- microbench.cu
 int run_microbench(bkr_ctx *ctx, int kind, int reps, double *result);
+// ---- probes.cu (kinds 10..22: result[0] = SM cycles, [1] = work units per SM, [2] = second work count)
+int run_probe(bkr_ctx *ctx, int kind, double *result);
 
 // ---- solver.cu
 int solver_block(bkr_ctx *ctx, double mass, int N, const double2 *B, double2 *X, double tol, int maxiter,

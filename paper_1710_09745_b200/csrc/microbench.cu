@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(MB_THREADS) mb_smem_kernel(double *out, int it
 
 int run_microbench(bkr_ctx *ctx, int kind, int reps, double *result)
 {
+    if (kind >= 10) return run_probe(ctx, kind, result);
     if (kind < 0 || kind > 9 || reps < 1 || !result) return BKR_EINVAL;
     const size_t BUF = (size_t)48 << 20;
     void *buf = nullptr;
@@ -255,5 +256,6 @@ int run_microbench(bkr_ctx *ctx, int kind, int reps, double *result)
     }
     result[0] = ms / reps;
     result[1] = units;
+    result[2] = 0.0;
     return BKR_OK;
 }
