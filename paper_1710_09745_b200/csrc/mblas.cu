@@ -52,6 +52,20 @@ __device__ __forceinline__ void mbar_arrive_rel(uint64_t *bar)
     asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
 }
 
+// The accumulator fragment of an 8 x 8 tile (lane 4 m + q holds row m, columns 2 q and 2 q + 1) -> the same entries of the
+// TRANSPOSED tile, by shuffles.  For a diagonal tile of X^dag X the product Xi^dag Xr is the transpose of Xr^dag Xi
+// (same products, same order of summation), so its DMMAs are not issued at all (the symmetry of the
+// reduction used inside a tile as well).  All 32 lanes must call it.
+__device__ __forceinline__ void frag_transpose(const double (&c)[2], double (&t)[2], int m, int q)
+{
+#pragma unroll
+    for (int r = 0; r < 2; r++) {
+        const int src = (2 * q + r) * 4 + (m >> 1);
+        const double v0 = __shfl_sync(0xffffffffu, c[0], src), v1 = __shfl_sync(0xffffffffu, c[1], src);
+        t[r] = (m & 1) ? v1 : v0;
+    }
+}
+
 template <typename Cx> __device__ __forceinline__ double2 sm_cx(const unsigned char *p)
 {
     const Cx v = *reinterpret_cast<const Cx *>(p);
@@ -439,7 +453,7 @@ gram_tma_kernel(size_t L, int N, RingPlan rp, const typename CxT<Real>::type *__
                         const double2 b = ALIAS ? xf[h][tj] : yf[h][tj];
                         dmma(acc[p][0], a.x, b.x);
                         dmma(acc[p][1], a.x, b.y);
-                        dmma(acc[p][2], a.y, b.x);
+                        if (!(ALIAS && ti == tj)) dmma(acc[p][2], a.y, b.x); // diagonal tile of X^dag X: the transpose of [1]
                         dmma(acc[p][3], a.y, b.y);
                     }
                 }
@@ -458,6 +472,7 @@ gram_tma_kernel(size_t L, int N, RingPlan rp, const typename CxT<Real>::type *__
             for (int ti = 0; ti < NXT; ti++) {
 #pragma unroll
                 for (int tj = HERM ? ti : 0; tj < NT; tj++, p++) {
+                    if (ALIAS && ti == tj) frag_transpose(acc[p][1], acc[p][2], m, q);
 #pragma unroll
                     for (int r = 0; r < 2; r++) {
                         const int i = 8 * (ti0 + ti) + m, j = 8 * tj + 2 * q + r;
@@ -919,7 +934,7 @@ update_gram_kernel(size_t L, int N, RingPlan rp, uint32_t off_red, const double2
                     for (int tj = ti; tj < NT; tj++, p++) {
                         dmma(acc[p][0], xf[ti].x, xf[tj].x);
                         dmma(acc[p][1], xf[ti].x, xf[tj].y);
-                        dmma(acc[p][2], xf[ti].y, xf[tj].x);
+                        if (ti != tj) dmma(acc[p][2], xf[ti].y, xf[tj].x); // diagonal tile: the transpose of [1] (frag_transpose)
                         dmma(acc[p][3], xf[ti].y, xf[tj].y);
                     }
             }
@@ -935,7 +950,8 @@ update_gram_kernel(size_t L, int N, RingPlan rp, uint32_t off_red, const double2
 #pragma unroll
             for (int ti = 0; ti < NT; ti++)
 #pragma unroll
-                for (int tj = ti; tj < NT; tj++, p++)
+                for (int tj = ti; tj < NT; tj++, p++) {
+                    if (ti == tj) frag_transpose(acc[p][1], acc[p][2], m, q);
 #pragma unroll
                     for (int r = 0; r < 2; r++) {
                         const int i = 8 * ti + m, j = 8 * tj + 2 * q + r;
@@ -946,6 +962,7 @@ update_gram_kernel(size_t L, int N, RingPlan rp, uint32_t off_red, const double2
                             red[i * N + j] = v;
                         }
                     }
+                }
         }
         asm volatile("bar.sync 1, %0;" ::"n"(CW * 32) : "memory");
     }
