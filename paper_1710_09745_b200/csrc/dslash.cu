@@ -169,6 +169,7 @@ dslash_kernel(Geom g, int N, int ntiles, const typename CxT<Real>::type *__restr
                     }
                 }
             }
+            asm volatile("fence.acq_rel.cta;" ::: "memory"); // the slot's loads are complete before it goes back (dslash_win.cu)
             __syncwarp();
             if ((tid & 31) == 0) mbar_arrive(&empty[slot]);
         }

@@ -313,6 +313,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                     for (int i = 0; i < T; i++) w[i] = lds_cx(wp + (i * 3 + b) * XH);
                 };
                 auto release_link = [&](int stage) {
+                    asm volatile("fence.acq_rel.cta;" ::: "memory"); // the slot's loads are complete before it goes back (dslash_win.cu)
                     __syncwarp();
                     if (lane == 0) {
                         uint64_t *bb = &lempty[stage & (RL - 1)];
@@ -400,6 +401,7 @@ __global__ void __launch_bounds__(ROW_THREADS, 1) dslash_row_kernel(const __grid
                 // rows the next tile does not need (v < TR (kl + 1) - 3), all of them after the last tile of the unit
                 {
                     const int new_rel = kl == UL - 1 ? rows_per_unit : (kl + 1) * TR;
+                    asm volatile("fence.acq_rel.cta;" ::: "memory");
                     __syncwarp();
                     if (lane == 0)
                         for (int cc = released; cc < new_rel; cc++) mbar_arrive(&wempty[(Q0 + cc) % WCH]);

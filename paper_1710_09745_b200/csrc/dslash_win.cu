@@ -329,7 +329,17 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
         const uint32_t stg_s = smem_addr(stg), win_s = smem_addr(win);
         int hslot = 0; // hop-stage ring position
         uint32_t hph = 0;
+        // A slot goes back to its producer when its last operands have been LOADED, a column or two before they are used -- so
+        // the arrival must not overtake those loads.  It does if nothing stops it: mbarrier.arrive is not queued behind
+        // earlier shared-memory loads of the warp, and when the load queue is congested (the xpay loads at the start of a
+        // tile) a refill -- ~700 cycles away on the idle 16^4 lattice -- landed before loads issued ahead of the arrive had
+        // executed: 2e-4 of the xpay launches there read one 32-byte sector of an operand of hop 8 from the chunk of hop
+        // 11, the next user of the slot (found by bit-exact reruns, decoded with a plane-indexed input; a data dependence of
+        // the barrier address on the loaded registers closes it as well, a dependence on the last column's registers alone
+        // moved the failure to the column before).  Hence a CTA-scope fence in front of every release: it completes the
+        // warp's outstanding loads first (0 mismatches in 2 x 10^6 launches; 3 % of the kernel's time).
         auto release_stage = [&](int s_) {
+            asm volatile("fence.acq_rel.cta;" ::: "memory");
             __syncwarp();
             if (C == 1) {
                 if (lane == 0) mbar_arrive(&hempty[s_]);
@@ -477,6 +487,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
                 // release the window chunks the next tile of this segment does not need
                 {
                     const int new_rel = (k == sg.y - 1) ? seg_hi + 1 : 2 * (k + 1) - HcL;
+                    asm volatile("fence.acq_rel.cta;" ::: "memory");
                     __syncwarp();
                     if (lane == 0) release_to(new_rel);
                     else

@@ -246,6 +246,7 @@ update_tma_kernel(size_t L, int N, RingPlan rp, const double2 *__restrict__ a, c
                 }
             }
         }
+        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
@@ -459,6 +460,7 @@ gram_tma_kernel(size_t L, int N, RingPlan rp, const typename CxT<Real>::type *__
                 }
             }
         }
+        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
@@ -733,6 +735,7 @@ pqx_update_kernel(size_t L, int N, Ring3 rp, const double2 *__restrict__ Si, con
                     }
             }
         }
+        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
@@ -941,6 +944,7 @@ update_gram_kernel(size_t L, int N, RingPlan rp, uint32_t off_red, const double2
         }
         // generic-proxy writes to the stage before the async-proxy (TMA) refill of the same shared memory
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
