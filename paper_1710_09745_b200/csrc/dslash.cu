@@ -338,11 +338,12 @@ int launch_dslash(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in,
             return rc;
         }
     }
-    // fp64 blocks of 22-24 and 30-32 rhs: ONE window launch, a cluster of 3 / 4 CTAs, every link read once per call
-    // (PAPER.md:224).  Measured at 32^3 x 64 against two launches of a cluster of 2 (links read twice): N = 24 2.21 vs
-    // 2.22 ms, N = 32 3.04 vs 2.88 ms -- the single pass is kept for the traffic it saves (BKR_TUNE_DSLASH_CHUNK = 2 splits).
-    if (!ctx->dslash_nblock && prec == BKR_F64 && N > 16 && 8 * ((N + 7) / 8) - N <= 2 && ctx->dslash_force != 0 &&
-        ctx->dslash_force != 2 && ctx->tune[BKR_TUNE_DSLASH_CHUNK] != 2) {
+    // fp64 blocks of 22-24 rhs: ONE window launch, a cluster of 3 CTAs, every link read once per call; as
+    // fast as 16 + rest (32^3 x 64, N = 24: 2.21 vs 2.22 ms).  A cluster of 4 (30-32 rhs) is not: 3.04 vs 2.88 ms there and
+    // 19.6 vs 16.0 ms at 48^3 x 96 for two launches of a cluster of 2, which read the links twice -- those blocks are
+    // split unless BKR_TUNE_DSLASH_CHUNK = 1 asks for the single pass (BKR_TUNE_DSLASH_CHUNK = 2 splits everything).
+    if (!ctx->dslash_nblock && prec == BKR_F64 && N > 16 && N <= 32 && 8 * ((N + 7) / 8) - N <= 2 && ctx->dslash_force != 0 &&
+        ctx->dslash_force != 2 && ctx->tune[BKR_TUNE_DSLASH_CHUNK] != 2 && (N <= 24 || ctx->tune[BKR_TUNE_DSLASH_CHUNK] == 1)) {
         const int rc = launch_dslash_win(ctx, out_parity, N, prec, in, out, xp, a, done);
         if (rc != 1) {
             ctx->dslash_variant = 1;

@@ -71,6 +71,7 @@ struct WinParams {
     int xover;  // 1: tiles do not start on x-row boundaries (64 % (X/2) != 0): x hops read the chunk below the tile
     int slim;   // 1: window without spare slots (chunks below the tile released after the y-3, y-1 hops)
     uint32_t off_win, off_bar;
+    uint32_t zero; // 0 at run time, unknown to the compiler: ties a barrier arrival to the registers of the loads it follows
 };
 
 // ---------------------------------------------------------------- PTX helpers (cluster, tensor TMA)
@@ -182,6 +183,8 @@ template <> __device__ __forceinline__ float2 lds_at<float2>(uint32_t addr, uint
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr + off));
     return v;
 }
+__device__ __forceinline__ uint32_t lo_bits(double v) { return (uint32_t)__double2loint(v); }
+__device__ __forceinline__ uint32_t lo_bits(float v) { return __float_as_uint(v); }
 __device__ __forceinline__ double shfl_x16(double v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
 __device__ __forceinline__ float shfl_x16(float v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
 
@@ -301,11 +304,10 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
         }
     } else {
         // ------------------------------------------------------------------ arithmetic warps
-        // Software pipeline: the operands of a COLUMN (3 link elements W_ab, a = 0..2, and the T vector elements of
-        // colour b) are loaded one column ahead of the 12 T FMAs that use them, into the register set (A or B) the
-        // running column does not use; the barrier probe is issued a column ahead as well.  Two hops = six columns bring
-        // the register roles back to where they started, so nothing is ever copied; the hop index is a compile-time
-        // constant (a runtime hop loop cost 280 non-FMA instructions per hop and warp, ncu).
+        // Software pipeline: the operands of a COLUMN are 3 link elements W_ab, a = 0..2, and the T vector elements of colour
+        // b, for 12 T FMAs.  Column 0 of a hop is loaded (register set A) during column 2 of the hop before, columns 1 and 2
+        // (sets B, C) at the start of the hop, the barrier probe of the next stage a column ahead; the hop index is a
+        // compile-time constant (a runtime hop loop cost 280 non-FMA instructions per hop and warp, ncu).
         asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(WIN_CONSUMER_REGS));
         const int set = lane >> 4;                     // 0: x/y hops from the window, 1: z/t hops from the stage ring
         const int sl = (warp & 3) * 16 + (lane & 15);  // site in tile
@@ -316,7 +318,7 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
         const uint32_t lkoff = (uint32_t)set * LSTAGE + (uint32_t)sl * (uint32_t)sizeof(Cx);
         const uint32_t ztoff = 2 * LSTAGE + (uint32_t)(sl >> 5) * WCHUNK + (uint32_t)(j0 * 3 * WIN_CHUNK + (sl & 31)) * (uint32_t)sizeof(Cx);
         const uint32_t woff = (uint32_t)(j0 * 3 * WIN_CHUNK) * (uint32_t)sizeof(Cx);
-        Cx uA[3], uB[3], vA[T], vB[T];
+        Cx uA[3], uB[3], uC[3], vA[T], vB[T], vC[T];
         // operand addresses are 32-bit shared-space integers: one base register per hop, immediate offsets per load
         auto load_u = [&](Cx(&u)[3], uint32_t lk, int b) {
 #pragma unroll
@@ -329,22 +331,29 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
         const uint32_t stg_s = smem_addr(stg), win_s = smem_addr(win);
         int hslot = 0; // hop-stage ring position
         uint32_t hph = 0;
-        // A slot goes back to its producer when its last operands have been LOADED, a column or two before they are used -- so
-        // the arrival must not overtake those loads.  It does if nothing stops it: mbarrier.arrive is not queued behind
-        // earlier shared-memory loads of the warp, and when the load queue is congested (the xpay loads at the start of a
-        // tile) a refill -- ~700 cycles away on the idle 16^4 lattice -- landed before loads issued ahead of the arrive had
-        // executed: 2e-4 of the xpay launches there read one 32-byte sector of an operand of hop 8 from the chunk of hop
-        // 11, the next user of the slot (found by bit-exact reruns, decoded with a plane-indexed input; a data dependence of
-        // the barrier address on the loaded registers closes it as well, a dependence on the last column's registers alone
-        // moved the failure to the column before).  Hence a CTA-scope fence in front of every release: it completes the
-        // warp's outstanding loads first (0 mismatches in 2 x 10^6 launches; 3 % of the kernel's time).
-        auto release_stage = [&](int s_) {
-            asm volatile("fence.acq_rel.cta;" ::: "memory");
+        // A slot goes back to its producer as soon as its operands are in registers, up to two columns before they are used
+        // -- so the arrival must not overtake those loads.  It does if nothing stops it: mbarrier.arrive is not queued
+        // behind earlier shared-memory loads of the warp, and when the load queue is congested (the xpay loads at the start of
+        // a tile) a refill -- ~700 cycles away on the idle 16^4 lattice -- landed before loads issued ahead of the arrive had
+        // executed: 2e-4 of the xpay launches there read one 32-byte sector of an operand of hop 8 from the chunk of hop 11,
+        // the next user of the slot (found by bit-exact reruns, decoded with a plane-indexed input).  The barrier ADDRESS
+        // is therefore computed from every register the stage was loaded into (all three columns), ANDed with p.zero = 0,
+        // which the compiler cannot know: the arrive cannot issue before the scoreboards of all those loads have cleared.
+        // (A dependence on the last column's registers alone moved the failure to the column before; a CTA-scope fence
+        // also closes it but waits for the xpay global loads as well.)
+        auto dep_of = [&](const Cx(&u)[3], const Cx(&v)[T]) -> uint32_t {
+            uint32_t d = lo_bits(u[0].x) | lo_bits(u[1].x) | lo_bits(u[2].x);
+#pragma unroll
+            for (int i = 0; i < T; i++) d |= lo_bits(v[i].x);
+            return d;
+        };
+        auto release_stage = [&](int s_, uint32_t dep) {
+            uint64_t *bb = reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(&hempty[s_]) + dep);
             __syncwarp();
             if (C == 1) {
-                if (lane == 0) mbar_arrive(&hempty[s_]);
+                if (lane == 0) mbar_arrive(bb);
             } else {
-                if (lane < C) mbar_arrive_remote(&hempty[s_], (uint32_t)lane);
+                if (lane < C) mbar_arrive_remote(bb, (uint32_t)lane);
             }
         };
         auto advance = [&]() {
@@ -374,9 +383,9 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
                 ex = el % Xh;
                 rowp = (el / Xh + zpar) & 1;
             }
-            auto release_to = [&](int new_rel) { // lane 0: give the chunks [released, new_rel) back to the window producer
+            auto release_to = [&](int new_rel, uint32_t dep) { // lane 0: give the chunks [released, new_rel) back to the window producer
                 for (; released < new_rel; released++) {
-                    mbar_arrive(&wempty[rl_slot]);
+                    mbar_arrive(reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(&wempty[rl_slot]) + dep));
                     if (++rl_slot == WCH) rl_slot = 0;
                 }
             };
@@ -429,67 +438,56 @@ dslash_win_kernel(const __grid_constant__ CUtensorMap tm_win, const WinParams p)
                 uint32_t lk = sb + lkoff, vp = set ? sb + ztoff : win_ptr(0);
                 load_u(uA, lk, 0);
                 load_v(vA, vp, 0);
-                auto hop_pair = [&](auto HC) {
+                // One hop: on entry register set A holds column 0; the loads of columns 1 and 2 are issued at once (sets B, C),
+                // so that by the end of column 0's FMAs every operand of the stage is in registers and the stage can go back
+                // to the producers without the arithmetic waiting for anything (release_stage).
+                auto hop = [&](auto HC) {
                     constexpr int h = decltype(HC)::value;
-                    // ---- hop h (column 0 is in register set A)
                     load_u(uB, lk, 1);
                     load_v(vB, vp, 1);
+                    load_u(uC, lk, 2);
+                    load_v(vC, vp, 2);
                     col_fma<Real, Cx, T>(acc, uA, vA);
-                    load_u(uA, lk, 2);
-                    load_v(vA, vp, 2);
-                    release_stage(hslot);
-                    advance();
-                    const uint32_t ok1 = mbar_try(&hfull[hslot], hph);
-                    const uint32_t sb1 = stg_s + (uint32_t)hslot * HSTAGE;
-                    const uint32_t vp1 = set ? sb1 + ztoff : win_ptr(h + 1);
-                    col_fma<Real, Cx, T>(acc, uB, vB);
-                    mbar_finish(ok1, &hfull[hslot], hph);
-                    const uint32_t lk1 = sb1 + lkoff;
-                    load_u(uB, lk1, 0);
-                    load_v(vB, vp1, 0);
-                    col_fma<Real, Cx, T>(acc, uA, vA);
-                    // ---- hop h + 1 (column 0 is in register set B)
-                    load_u(uA, lk1, 1);
-                    load_v(vA, vp1, 1);
-                    col_fma<Real, Cx, T>(acc, uB, vB);
-                    load_u(uB, lk1, 2);
-                    load_v(vB, vp1, 2);
-                    release_stage(hslot);
-                    if (h == 0 && p.slim) {
+                    const uint32_t dep = (dep_of(uA, vA) | dep_of(uB, vB) | dep_of(uC, vC)) & p.zero;
+                    release_stage(hslot, dep);
+                    if (h == 1 && p.slim) {
                         // hops 0, 1 are y-3, y-1 (common.cuh): the chunks below the tile are dead from here on and go back
                         // to the window producer, which loads the next tile's upper chunks into them
                         const int new_rel = 2 * k - p.xover; // x neighbours reach 2 sites below a tile that starts mid-row
-                        // (after the __syncwarp of release_stage: every lane has issued its last read; every lane keeps the counters)
-                        if (lane == 0) release_to(new_rel);
+                        if (lane == 0) release_to(new_rel, dep);
                         else
                             for (; released < new_rel; released++)
                                 if (++rl_slot == WCH) rl_slot = 0;
                     }
                     advance();
-                    if constexpr (h < 6) {
-                        const uint32_t ok2 = mbar_try(&hfull[hslot], hph);
+                    if constexpr (h < 7) {
+                        const uint32_t ok = mbar_try(&hfull[hslot], hph);
                         sb = stg_s + (uint32_t)hslot * HSTAGE;
-                        vp = set ? sb + ztoff : win_ptr(h + 2);
-                        col_fma<Real, Cx, T>(acc, uA, vA);
-                        mbar_finish(ok2, &hfull[hslot], hph);
+                        vp = set ? sb + ztoff : win_ptr(h + 1);
+                        col_fma<Real, Cx, T>(acc, uB, vB);
+                        mbar_finish(ok, &hfull[hslot], hph);
                         lk = sb + lkoff;
                         load_u(uA, lk, 0);
                         load_v(vA, vp, 0);
                     } else {
-                        col_fma<Real, Cx, T>(acc, uA, vA);
+                        col_fma<Real, Cx, T>(acc, uB, vB);
                     }
-                    col_fma<Real, Cx, T>(acc, uB, vB);
+                    col_fma<Real, Cx, T>(acc, uC, vC);
+                    return dep;
                 };
-                hop_pair(std::integral_constant<int, 0>{});
-                hop_pair(std::integral_constant<int, 2>{});
-                hop_pair(std::integral_constant<int, 4>{});
-                hop_pair(std::integral_constant<int, 6>{});
+                hop(std::integral_constant<int, 0>{});
+                hop(std::integral_constant<int, 1>{});
+                hop(std::integral_constant<int, 2>{});
+                hop(std::integral_constant<int, 3>{});
+                hop(std::integral_constant<int, 4>{});
+                hop(std::integral_constant<int, 5>{});
+                hop(std::integral_constant<int, 6>{});
+                const uint32_t dep_last = hop(std::integral_constant<int, 7>{});
                 // release the window chunks the next tile of this segment does not need
                 {
                     const int new_rel = (k == sg.y - 1) ? seg_hi + 1 : 2 * (k + 1) - HcL;
-                    asm volatile("fence.acq_rel.cta;" ::: "memory");
                     __syncwarp();
-                    if (lane == 0) release_to(new_rel);
+                    if (lane == 0) release_to(new_rel, dep_last); // (issued after hop 15's release: every window load has returned)
                     else
                         for (; released < new_rel; released++)
                             if (++rl_slot == WCH) rl_slot = 0;
@@ -652,6 +650,7 @@ static int launch_win_x(bkr_ctx *ctx, int parity, int N, int prec, const void *i
     p.segs = ctx->win_segs;
     p.nseg = ctx->win_nseg;
     p.done = done;
+    p.zero = 0;
 
     auto kern = dslash_win_kernel<Real, T, C, XP>;
     static int max_clusters = -1, attr_dev = -1; // per instantiation; the shared-memory opt-in is per device
