@@ -87,6 +87,7 @@ struct RingPlan {
     int R, nstg;
     uint32_t rs_a, rs_b, off_b, stage_bytes, off_ring; // off_ring: start of the ring in dynamic shared memory
     size_t smem;
+    uint32_t zero; // 0 at run time, unknown to the compiler (ties a barrier arrival to registers, gram_tma_kernel)
 };
 
 // pad: the residue (mod 128 bytes) the chunk stride must have so that fragment loads are conflict-free
@@ -101,6 +102,7 @@ static RingPlan plan_ring(size_t L, size_t fixed, int min_stages, int nchunk_a, 
     fixed = (fixed + 127) / 128 * 128;
     for (int R = 1024; R >= 64; R /= 2) {
         RingPlan p;
+        p.zero = 0;
         p.R = R;
         p.rs_a = (uint32_t)(R * esize_a + pad_a);
         p.rs_b = (uint32_t)(R * esize_b + pad_b);
@@ -246,7 +248,8 @@ update_tma_kernel(size_t L, int N, RingPlan rp, const double2 *__restrict__ a, c
                 }
             }
         }
-        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
+        // (the stores above take their data from everything the stage was loaded for: a release cannot move above them,
+        // so the loads have returned -- no fence needed here, dslash_win.cu has the story)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
@@ -460,9 +463,17 @@ gram_tma_kernel(size_t L, int N, RingPlan rp, const typename CxT<Real>::type *__
                 }
             }
         }
-        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
+        // The stage goes back when its fragments have been consumed: the barrier address depends on every accumulator (all
+        // of them took a DMMA from the last k-step), so the arrive cannot issue before those loads have returned
+        // (dslash_win.cu has the story; a CTA-scope fence here cost 7 %).
+        uint32_t dep = 0;
+#pragma unroll
+        for (int p = 0; p < NP; p++)
+#pragma unroll
+            for (int c = 0; c < 4; c++) dep |= (uint32_t)__double2loint(acc[p][c][0]) | (uint32_t)__double2loint(acc[p][c][1]);
+        dep &= rp.zero;
         __syncwarp();
-        if (lane == 0) mbar_arrive_rel(&empty[s]);
+        if (lane == 0) mbar_arrive_rel(reinterpret_cast<uint64_t *>(reinterpret_cast<unsigned char *>(&empty[s]) + dep));
     }
 
     // fixed-order reduction over the consumer warps of the CTA, then one partial per CTA.  Named barrier 1 over the
@@ -735,7 +746,8 @@ pqx_update_kernel(size_t L, int N, Ring3 rp, const double2 *__restrict__ Si, con
                     }
             }
         }
-        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
+        // (the stores above take their data from everything the stage was loaded for: a release cannot move above them,
+        // so the loads have returned -- no fence needed here, dslash_win.cu has the story)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
@@ -944,7 +956,8 @@ update_gram_kernel(size_t L, int N, RingPlan rp, uint32_t off_red, const double2
         }
         // generic-proxy writes to the stage before the async-proxy (TMA) refill of the same shared memory
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("fence.acq_rel.cta;" ::: "memory"); // the stage's loads are complete before it goes back (dslash_win.cu)
+        // (the stores above take their data from everything the stage was loaded for: a release cannot move above them,
+        // so the loads have returned -- no fence needed here, dslash_win.cu has the story)
         __syncwarp();
         if (lane == 0) mbar_arrive_rel(&empty[s]);
     }
