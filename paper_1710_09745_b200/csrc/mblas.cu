@@ -18,39 +18,7 @@
 // because one DMMA replaces 8 DFMAs per lane and needs 2 operand registers for 8 FMAs.  A complex product is 4 real
 // DMMAs.  All accumulation is fp64 whatever the storage precision.  Reductions finish in a fixed order (no
 // floating-point atomics): results are bit-reproducible.
-#include "common.cuh"
-#include "tma.cuh"
-
-#include <stdlib.h>
-#include <string.h>
-
-static const int MB_SMEM_BUDGET = 216 * 1024; // of the 227 KB a CTA may opt in to
-static const int MB_MAX_STAGES = 8;
-
-__device__ __forceinline__ void dmma(double (&c)[2], double a, double b)
-{
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(c[0]), "+d"(c[1])
-        : "d"(a), "d"(b));
-}
-
-// mbarrier wait that is also a compiler barrier for memory: the plain shared-memory reads of a stage must not move
-// above it
-__device__ __forceinline__ void mbar_wait_acq(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(smem_addr(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void mbar_arrive_rel(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
-}
+#include "mblas.cuh"
 
 // The accumulator fragment of an 8 x 8 tile (lane 4 m + q holds row m, columns 2 q and 2 q + 1) -> the same entries of the
 // TRANSPOSED tile, by shuffles.  For a diagonal tile of X^dag X the product Xi^dag Xr is the transpose of Xr^dag Xi
@@ -64,63 +32,6 @@ __device__ __forceinline__ void frag_transpose(const double (&c)[2], double (&t)
         const double v0 = __shfl_sync(0xffffffffu, c[0], src), v1 = __shfl_sync(0xffffffffu, c[1], src);
         t[r] = (m & 1) ? v1 : v0;
     }
-}
-
-template <typename Cx> __device__ __forceinline__ double2 sm_cx(const unsigned char *p)
-{
-    const Cx v = *reinterpret_cast<const Cx *>(p);
-    return make_double2((double)v.x, (double)v.y);
-}
-template <typename Cx> __device__ __forceinline__ void st_cx(Cx *p, double re, double im);
-template <> __device__ __forceinline__ void st_cx<double2>(double2 *p, double re, double im)
-{
-    __stcs(p, make_double2(re, im));
-}
-template <> __device__ __forceinline__ void st_cx<float2>(float2 *p, double re, double im)
-{
-    __stcs(p, make_float2((float)re, (float)im));
-}
-
-// Ring geometry shared by host and device.  A stage holds `nchunk_a` chunks of stride rs_a and `nchunk_b` chunks of
-// stride rs_b (bytes); a chunk is R consecutive rows of one vector.
-struct RingPlan {
-    int R, nstg;
-    uint32_t rs_a, rs_b, off_b, stage_bytes, off_ring; // off_ring: start of the ring in dynamic shared memory
-    size_t smem;
-    uint32_t zero; // 0 at run time, unknown to the compiler (ties a barrier arrival to registers, gram_tma_kernel)
-};
-
-// pad: the residue (mod 128 bytes) the chunk stride must have so that fragment loads are conflict-free
-// Policy (measured, 32^4): a stage costs ~600 cycles of fixed overhead plus ~40 per bulk copy,
-// so R is the largest power of two that still leaves `min_stages` stages in the ring (3 for the reductions, 4 for the
-// updates, whose consumers also write) and gives every SM at least two row tiles.
-static RingPlan plan_ring(size_t L, size_t fixed, int min_stages, int nchunk_a, int esize_a, int pad_a, int nchunk_b,
-                          int esize_b, int pad_b)
-{
-    RingPlan best;
-    memset(&best, 0, sizeof(best));
-    fixed = (fixed + 127) / 128 * 128;
-    for (int R = 1024; R >= 64; R /= 2) {
-        RingPlan p;
-        p.zero = 0;
-        p.R = R;
-        p.rs_a = (uint32_t)(R * esize_a + pad_a);
-        p.rs_b = (uint32_t)(R * esize_b + pad_b);
-        p.off_b = ((uint32_t)nchunk_a * p.rs_a + 127) / 128 * 128;
-        p.stage_bytes = (p.off_b + (uint32_t)nchunk_b * p.rs_b + 127) / 128 * 128;
-        p.off_ring = (uint32_t)fixed;
-        int n = (int)((MB_SMEM_BUDGET - fixed) / p.stage_bytes);
-        if (n > MB_MAX_STAGES) n = MB_MAX_STAGES;
-        p.nstg = n;
-        p.smem = fixed + (size_t)n * p.stage_bytes;
-        bool ok = n >= min_stages && (L + R - 1) / R >= (size_t)2 * BKR_NUM_SMS;
-        if (ok || R == 64) {
-            if (n < 2) p.nstg = 0; // does not fit at all (cannot happen for N <= 32)
-            best = p;
-            break;
-        }
-    }
-    return best;
 }
 
 // ------------------------------------------------------------------------------------------ streaming update
@@ -336,6 +247,7 @@ int launch_block_update(bkr_ctx *ctx, int N, int precZ, int precW, const double2
         }
         return BKR_OK;
     }
+    if (precZ == BKR_F32 && precW == BKR_F32 && f32_tf32_update(ctx)) return launch_block_update_tf32(ctx, N, a, C, W, Z, done, tri);
     if (precZ == BKR_F64 && precW == BKR_F64) return launch_update_t<double, double>(ctx, N, a, C, W, Z, done, tri);
     if (precZ == BKR_F64 && precW == BKR_F32) return launch_update_t<double, float>(ctx, N, a, C, W, Z, done, tri);
     if (precZ == BKR_F32 && precW == BKR_F32) return launch_update_t<float, float>(ctx, N, a, C, W, Z, done, tri);
@@ -550,6 +462,7 @@ int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const voi
                          const int *done)
 {
     const size_t L = (size_t)ctx->g.Vh * 3;
+    if (prec == BKR_F32 && f32_tf32_gram(ctx, N, hermitian)) return launch_gram_partials_tf32(ctx, N, X, Y, hermitian, num_partials, done);
     BKR_TRY(ensure_partials(ctx, (size_t)2 * BKR_NUM_SMS * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
     const int NT = (N + 7) / 8;
 #define GRAM_NT(Real)                                                                    \
@@ -574,12 +487,6 @@ int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const voi
 //     X  += P Wm      if flags->xpend   (Wm = beta C of the previous l.9; X fp64, in place)
 // 6 block passes.  Same ring, fragment layouts and DMMA tiles as update_tma_kernel; a stage holds R rows of Q' and P
 // (A-fragment layout) and of X (accumulator layout).
-struct Ring3 {
-    int R, nstg;
-    uint32_t rs_p, rs_q, rs_x, off_q, off_x, stage_bytes, off_ring;
-    size_t smem;
-};
-
 template <typename RealP, int NTJ, int NIS, int CW>
 __global__ void __launch_bounds__((CW + 1) * 32, 1)
 pqx_update_kernel(size_t L, int N, Ring3 rp, const double2 *__restrict__ Si, const double2 *__restrict__ Sd,
@@ -760,23 +667,7 @@ static int pqx_go(bkr_ctx *ctx, size_t L, int N, const double2 *Si, const double
     typedef typename CxT<RealP>::type CxP;
     constexpr int CW = 8;
     const size_t fixed = (128 + (size_t)6 * NIS * NTJ * 32 * sizeof(double) + 127) / 128 * 128;
-    Ring3 rp;
-    memset(&rp, 0, sizeof(rp));
-    for (int R = 512; R >= 32; R /= 2) {
-        rp.R = R;
-        rp.rs_p = (uint32_t)(R * sizeof(CxP) + 32);
-        rp.rs_q = (uint32_t)(R * sizeof(CxP) + 32); // Q' is an A operand here
-        rp.rs_x = (uint32_t)(R * sizeof(double2) + 16);
-        rp.off_q = ((uint32_t)N * rp.rs_p + 127) / 128 * 128;
-        rp.off_x = (rp.off_q + (uint32_t)N * rp.rs_q + 127) / 128 * 128;
-        rp.stage_bytes = (rp.off_x + (uint32_t)N * rp.rs_x + 127) / 128 * 128;
-        rp.off_ring = (uint32_t)fixed;
-        int n = (int)((MB_SMEM_BUDGET - fixed) / rp.stage_bytes);
-        if (n > MB_MAX_STAGES) n = MB_MAX_STAGES;
-        rp.nstg = n;
-        rp.smem = fixed + (size_t)n * rp.stage_bytes;
-        if ((n >= 4 && (L + R - 1) / R >= (size_t)2 * BKR_NUM_SMS) || R == 32) break;
-    }
+    const Ring3 rp = plan_ring3(L, N, fixed, (int)sizeof(CxP));
     if (rp.nstg < 2) return BKR_EINVAL;
     const size_t ntiles = (L + rp.R - 1) / rp.R;
     const unsigned grid = (unsigned)(ntiles < (size_t)BKR_NUM_SMS ? ntiles : (size_t)BKR_NUM_SMS);
@@ -815,6 +706,7 @@ int launch_pqx_update(bkr_ctx *ctx, int N, int prec, const double2 *Sinv, const 
                       const void *P, void *Pn, double2 *X, const SolverFlags *flags)
 {
     if (prec == BKR_F64) return launch_pqx_t<double>(ctx, N, Sinv, Sdag, Wm, Q, P, Pn, X, flags);
+    if (N <= 16 && f32_tf32_update(ctx)) return launch_pqx_update_tf32(ctx, N, Sinv, Sdag, Wm, Q, P, Pn, X, flags);
     return launch_pqx_t<float>(ctx, N, Sinv, Sdag, Wm, Q, P, Pn, X, flags);
 }
 
@@ -1017,6 +909,7 @@ int launch_update_gram(bkr_ctx *ctx, int N, int prec, const double2 *a, const vo
                        const int *done)
 {
     const size_t L = (size_t)ctx->g.Vh * 3;
+    if (prec == BKR_F32 && N <= 16 && f32_tf32_update(ctx)) return launch_update_gram_tf32(ctx, N, a, C, W, Z, num_partials, done);
 #define UG_GO(Real, NT_, NIS_) return update_gram_go<Real, NT_, NIS_>(ctx, L, N, a, C, W, Z, num_partials, done)
 #define UG_SW(Real)                  \
     switch ((N + 3) / 4) {           \

@@ -1,0 +1,179 @@
+"""GPU parity of the split-TF32 multi-BLAS for fp32 blocks (csrc/mblas_tf32.cu, reading U25)
+against the oracle's plain fp64 loops (eq. 3 / eq. 4) on the same fp32-rounded inputs, element by element.
+
+Error budget: a split product drops x_lo y_lo and truncates the low parts, ~2^-21 per product; a
+reduction keeps fp32 partial sums over 64 rows and fp64 beyond.  Measured 1e-7 .. 7e-7 of the largest entry; asserted
+<= 2e-6 for reductions and <= 1e-5 (the fp32 storage tolerance of the other tests) for updates.  The FP64 tensor path
+(F32_MATH_FP64) stays exact to 1e-13 on the same inputs and is checked beside it.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from tests import helpers as H
+
+pytestmark = pytest.mark.gpu
+TOL_GRAM, TOL32 = 2e-6, 1e-5
+
+
+def _round32(a):
+    return a.astype(np.complex64).astype(np.complex128)
+
+
+def _ctx(dims, seed):
+    from paper_1710_09745_b200 import binding
+    fat, lng = H.np_links(dims, "random", seed=seed)
+    ctx = binding.Context(dims)
+    ctx.load_links(torch.from_numpy(fat).cuda(), torch.from_numpy(lng).cuda(), also_f32=True)
+    return dims, ctx
+
+
+@pytest.fixture(scope="module")
+def lat():
+    return _ctx((4, 6, 8, 10), 51)  # L = 2880 rows: several 16-row units per warp, one ring stage per CTA
+
+
+@pytest.fixture(scope="module")
+def lat_ragged():
+    return _ctx((6, 6, 6, 6), 52)  # L = 1944 = 121 x 16 + 8: the last unit of a block has 8 rows
+
+
+@pytest.fixture(scope="module")
+def lat_wrap():
+    return _ctx((16, 16, 16, 16), 53)  # L = 98304 rows: the ring wraps (more row tiles than stages per CTA)
+
+
+def _tf32(ctx):
+    from paper_1710_09745_b200 import binding
+
+    class _Mode:
+        def __enter__(self):
+            ctx.set_f32_math(binding.F32_MATH_TF32)
+
+        def __exit__(self, *a):
+            ctx.set_f32_math(binding.F32_MATH_AUTO)
+    return _Mode()
+
+
+@pytest.mark.parametrize("N", [1, 4, 7, 8, 12, 16, 20, 24, 32])
+@pytest.mark.parametrize("kind", ["general", "hermitian_two_blocks", "aliased"])
+def test_gram_split_tf32(lat, N, kind):
+    """K = X^dag Y (eq. 4) on the TF32 path at every tile count, all three instances"""
+    from paper_1710_09745_b200 import binding
+    dims, ctx = lat
+    X = _round32(H.np_sources(dims, N, 5100 + N))
+    Y = X if kind == "aliased" else _round32(H.np_sources(dims, N, 5200 + N))
+    Xd = ctx.pack(torch.from_numpy(X).cuda(), binding.F32)
+    Yd = Xd if kind == "aliased" else ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
+    with _tf32(ctx):
+        K = ctx.gram(N, Xd, Yd, hermitian=(kind != "general"), prec=binding.F32).cpu().numpy()
+    want = oracle.gram(X, Y)
+    scale = np.abs(want).max()
+    if kind == "hermitian_two_blocks":  # a general Y: only the upper triangle and the real diagonal are defined
+        iu = np.triu_indices(N, 1)
+        assert N == 1 or np.abs(K[iu] - want[iu]).max() <= TOL_GRAM * scale
+        assert np.abs(K.diagonal().real - want.diagonal().real).max() <= TOL_GRAM * scale
+    else:
+        assert np.abs(K - want).max() <= TOL_GRAM * scale
+    if kind == "aliased":
+        assert np.abs(K - K.conj().T).max() == 0.0 and np.abs(np.diag(K).imag).max() == 0.0
+
+
+@pytest.mark.parametrize("N", [5, 16, 32])
+def test_gram_split_tf32_ragged_and_wrapping(lat_ragged, lat_wrap, N):
+    from paper_1710_09745_b200 import binding
+    for dims, ctx in (lat_ragged, lat_wrap):
+        X, Y = _round32(H.np_sources(dims, N, 5300 + N)), _round32(H.np_sources(dims, N, 5400 + N))
+        Xd, Yd = ctx.pack(torch.from_numpy(X).cuda(), binding.F32), ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
+        with _tf32(ctx):
+            K = ctx.gram(N, Xd, Yd, hermitian=False, prec=binding.F32).cpu().numpy()
+            Ka = ctx.gram(N, Xd, Xd, hermitian=True, prec=binding.F32).cpu().numpy()
+        want, wanta = oracle.gram(X, Y), oracle.gram(X, X)
+        assert np.abs(K - want).max() <= TOL_GRAM * np.abs(want).max()
+        assert np.abs(Ka - wanta).max() <= TOL_GRAM * np.abs(wanta).max()
+
+
+@pytest.mark.parametrize("N", [1, 4, 7, 8, 12, 16, 20, 24, 32])
+@pytest.mark.parametrize("tri", [0, 1, 2])
+def test_block_update_split_tf32(lat, lat_ragged, N, tri):
+    """Z = C + W a (eq. 3) with general / upper / lower triangular a, and without C"""
+    from paper_1710_09745_b200 import binding
+    rng = np.random.default_rng(700 + 3 * N + tri)
+    a = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    a = np.triu(a) if tri == 1 else np.tril(a) if tri == 2 else a
+    # a skipped coefficient tile must not be read: poison the zero side of the triangle where whole 8 x 8 tiles lie on it
+    ap = a.copy()
+    for i in range(N):
+        for j in range(N):
+            if (tri == 1 and i // 8 > j // 8) or (tri == 2 and i // 8 < j // 8):
+                ap[i, j] = 1e30
+    for dims, ctx in (lat, lat_ragged):
+        W, C = _round32(H.np_sources(dims, N, 5500 + N)), _round32(H.np_sources(dims, N, 5600 + N))
+        Wd, Cd = ctx.pack(torch.from_numpy(W).cuda(), binding.F32), ctx.pack(torch.from_numpy(C).cuda(), binding.F32)
+        with _tf32(ctx):
+            Zd = ctx.block_update(N, torch.from_numpy(ap).cuda(), Cd, Wd, ctx.empty_native(N, binding.F32), binding.F32, binding.F32, tri)
+            Z0 = ctx.block_update(N, torch.from_numpy(ap).cuda(), None, Wd, ctx.empty_native(N, binding.F32), binding.F32, binding.F32, tri)
+        assert H.relerr_inf(ctx.unpack(Zd, N, binding.F32).cpu().numpy(), oracle.block_axpy(a, W, C)) <= TOL32
+        assert H.relerr_inf(ctx.unpack(Z0, N, binding.F32).cpu().numpy(), oracle.block_axpy(a, W, np.zeros_like(W))) <= TOL32
+
+
+@pytest.mark.parametrize("N", [3, 8, 13, 16])
+def test_fused_update_gram_split_tf32(lat, lat_ragged, lat_wrap, N):
+    """Alg. 1 l.11 fused with stage 1 of H = Q'^dag Q': H is the Gram matrix of the stored block"""
+    from paper_1710_09745_b200 import binding
+    rng = np.random.default_rng(800 + N)
+    a = rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    for dims, ctx in (lat, lat_ragged, lat_wrap):
+        X, Y = _round32(H.np_sources(dims, N, 5700 + N)), _round32(H.np_sources(dims, N, 5800 + N))
+        Xd, Yd = ctx.pack(torch.from_numpy(X).cuda(), binding.F32), ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
+        with _tf32(ctx):
+            K = ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd, prec=binding.F32).cpu().numpy()
+        got = ctx.unpack(Yd, N, binding.F32).cpu().numpy()
+        assert H.relerr_inf(got, oracle.block_axpy(a, X, Y)) <= TOL32
+        wantK = oracle.gram(got, got)
+        assert np.abs(K - wantK).max() <= TOL_GRAM * np.abs(wantK).max()
+        assert np.abs(K - K.conj().T).max() == 0.0 and np.abs(np.diag(K).imag).max() == 0.0
+
+
+@pytest.mark.parametrize("N", [3, 8, 13, 16])
+def test_fused_qpx_update_split_tf32(lat, lat_ragged, lat_wrap, N):
+    """Q = Q' S^-1, P = Q + P S^dag, X += P W in one pass, fp32 Q and P, fp64 X"""
+    from paper_1710_09745_b200 import binding
+    rng = np.random.default_rng(900 + N)
+    full = lambda: rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N))
+    Sinv, Sdag, Wm = np.triu(full()), np.tril(full()), full()
+    for dims, ctx in (lat, lat_ragged, lat_wrap):
+        Q, P = (_round32(H.np_sources(dims, N, 5900 + 10 * k + N)) for k in range(2))
+        X = H.np_sources(dims, N, 5930 + N)
+        Qd, Pd = (ctx.pack(torch.from_numpy(v).cuda(), binding.F32) for v in (Q, P))
+        Xd = ctx.pack(torch.from_numpy(X).cuda())
+        Pn = torch.empty_like(Pd)
+        with _tf32(ctx):
+            ctx.block_qpx_update(N, *(torch.from_numpy(m).cuda() for m in (Sinv, Sdag, Wm)), Qd, Pd, Pn, Xd, prec=binding.F32)
+        Qn = oracle.block_axpy(Sinv, Q, np.zeros_like(Q))
+        assert H.relerr_inf(ctx.unpack(Qd, N, binding.F32).cpu().numpy(), Qn) <= TOL32
+        assert H.relerr_inf(ctx.unpack(Pn, N, binding.F32).cpu().numpy(), oracle.block_axpy(Sdag, P, Qn)) <= TOL32
+        assert H.relerr_inf(ctx.unpack(Xd, N).cpu().numpy(), oracle.block_axpy(Wm, P, X)) <= TOL_GRAM
+
+
+def test_mixed_solver_same_iterations_on_both_tensor_paths(lat_wrap):
+    """the fp32-inner blockCGrQ (Alg. 3) with split-TF32 multi-BLAS against the same solve with exact FP64 tensor products:
+    both reach the tolerance (true residual recomputed by the oracle), iteration counts within 2 %"""
+    from paper_1710_09745_b200 import binding
+    dims, ctx = lat_wrap
+    fat, lng = H.np_links(dims, "random", seed=53)
+    N = 16
+    B = H.np_sources(dims, N, 6100)
+    Bd = torch.from_numpy(B).cuda()
+    out = {}
+    for mode in (binding.F32_MATH_FP64, binding.F32_MATH_AUTO):
+        ctx.set_f32_math(mode)
+        try:
+            X, rr, st = ctx.solve_block(0.05, Bd, tol=1e-10, inner_prec=binding.F32, delta=0.1)
+        finally:
+            ctx.set_f32_math(binding.F32_MATH_AUTO)
+        assert st["status"] == 0
+        assert oracle.true_relres(dims, fat, lng, 0.05, B, X.cpu().numpy()).max() <= 1e-10
+        out[mode] = st["iters"]
+    assert abs(out[binding.F32_MATH_AUTO] - out[binding.F32_MATH_FP64]) <= max(2, 0.02 * out[binding.F32_MATH_FP64])
