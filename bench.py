@@ -209,7 +209,8 @@ PROBE_KINDS = [(10, "lds128_conflict_free_B_per_clk_sm", "bytes"), (11, "lds128_
                (16, "dfma_with_4_lds128_per_64_per_clk_sm", "dfma"), (17, "dfma_with_8_lds128_per_64_per_clk_sm", "dfma"),
                (18, "dry_stencil_T4_8warps_dfma_per_clk_sm", "dfma"), (19, "dry_stencil_T8_4warps_dfma_per_clk_sm", "dfma"),
                (20, "dry_stencil_T8_8warps_dfma_per_clk_sm", "dfma"),
-               (21, "tma_9KB_issue_interval_clk_one_lane", "interval"), (22, "tma_9KB_round_trip_clk_idle_l2", "interval")]
+               (21, "tma_9KB_issue_interval_clk_one_lane", "interval"), (22, "tma_9KB_round_trip_clk_idle_l2", "interval"),
+               (23, "mma_sync_tf32_m16n8k8_flop_per_clk_sm", "flop")]
 
 
 def run_probes(ctx):
@@ -633,9 +634,16 @@ def run_sweep(args):
     ctx = binding.Context(dims)
     ctx.load_links(fat, lng, also_f32=True)
     del fat, lng
-    for prec, pname in ((binding.F64, "f64"), (binding.F32, "f32")):
-        for N in (1, 2, 4, 8, 16, 24, 32):
+    # third pass: fp32 blocks with the split-TF32 multi-BLAS (BKR_TUNE_F32_MATH = 1; not the default).
+    # Its "frac_roofline" still divides by the FP64 FMA peak: read frac_hbm there.
+    for prec, pname, math in ((binding.F64, "f64", binding.F32_MATH_FP64), (binding.F32, "f32", binding.F32_MATH_FP64),
+                              (binding.F32, "f32_tf32", binding.F32_MATH_TF32)):
+        ctx.set_f32_math(math)
+        for N in ((1, 2, 4, 8, 16, 24, 32) if pname != "f32_tf32" else (8, 16, 24, 32)):
             k = kernel_numbers(torch, ctx, binding, dims, N, prec, reps=args.steps, warmup=3, hbm=hbm)
+            if pname == "f32_tf32":
+                for kn in ("dslash", "dslash_xpay"):
+                    k.pop(kn, None)
             row = {"sweep": name, "dtype": pname, "N": N}
             for kn, v in k.items():
                 row[kn] = {a: (round(b, 4) if isinstance(b, float) else b) for a, b in v.items()}

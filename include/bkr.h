@@ -216,8 +216,9 @@ enum {
     BKR_TUNE_DSLASH_CHUNK = 1,    /* 1 = never split a block into chunks of 16 / 8 rhs; 2 = always split blocks > 16 rhs   */
     BKR_TUNE_WIN_SEGLEN = 2,      /* 64-site tiles per segment (default 8)                                                */
     BKR_TUNE_WIN_SLIM = 3,        /* 2 = keep spare window slots instead of releasing the lower halo early                */
-    BKR_TUNE_F32_MATH = 4,        /* multi-BLAS on fp32 blocks: 0 = split-TF32 or FP64 tensor products, whichever measured   */
-                                  /* faster (default), 1 = FP64 DMMA everywhere (exact products), 2 = split-TF32 everywhere */
+    BKR_TUNE_F32_MATH = 4,        /* multi-BLAS on fp32 blocks: 0 = FP64 tensor products, exact (default); 1 = split-TF32   */
+                                  /* everywhere it exists (faster per call, ~3e-7 errors: more solver iterations);          */
+                                  /* 2 = split-TF32 updates only; 3 = split-TF32 reductions only                            */
     BKR_TUNE_COUNT = 16
 };
 enum {

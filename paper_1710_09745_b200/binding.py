@@ -19,8 +19,8 @@ MAX_N = 32
 OPT_L2_BUDGET_MB, OPT_ROW_UNIT_TILES, OPT_ROW_VEC_POLICY, OPT_ABLATION = 0, 1, 2, 3
 ABL_UNFUSED_UPDATES, ABL_UNFUSED_GRAM, ABL_VECTOR_BLAS, ABL_VECTOR_DSLASH = 1, 2, 4, 8
 OPT_TUNE = 16  # + BKR_TUNE_* (bkr.h)
-TUNE_F32_MATH = 4  # multi-BLAS on fp32 blocks: 0 automatic, 1 FP64 DMMA everywhere, 2 split-TF32 everywhere
-F32_MATH_AUTO, F32_MATH_FP64, F32_MATH_TF32 = 0, 1, 2
+TUNE_F32_MATH = 4  # multi-BLAS on fp32 blocks: 0 FP64 tensor products (default), 1 split-TF32, 2 / 3 TF32 updates / reductions only
+F32_MATH_FP64, F32_MATH_TF32, F32_MATH_TF32_UPDATES, F32_MATH_TF32_GRAM = 0, 1, 2, 3
 
 SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash", "bkr_dslash_xpay",
@@ -350,7 +350,7 @@ class Context:
         self._check(lib().bkr_set_option(self._h, int(option), int(value)), "bkr_set_option")
 
     def set_f32_math(self, mode):
-        """tensor path of the multi-BLAS on fp32 blocks (bkr.h BKR_TUNE_F32_MATH): F32_MATH_AUTO / _FP64 / _TF32"""
+        """tensor path of the multi-BLAS on fp32 blocks (bkr.h BKR_TUNE_F32_MATH): F32_MATH_FP64 (default) / _TF32 / _TF32_UPDATES / _TF32_GRAM"""
         self.set_option(OPT_TUNE + TUNE_F32_MATH, mode)
 
     def set_dslash_variant(self, variant):

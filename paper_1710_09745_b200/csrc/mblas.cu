@@ -462,7 +462,7 @@ int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const voi
                          const int *done)
 {
     const size_t L = (size_t)ctx->g.Vh * 3;
-    if (prec == BKR_F32 && f32_tf32_gram(ctx, N, hermitian)) return launch_gram_partials_tf32(ctx, N, X, Y, hermitian, num_partials, done);
+    if (prec == BKR_F32 && f32_tf32_gram(ctx)) return launch_gram_partials_tf32(ctx, N, X, Y, hermitian, num_partials, done);
     BKR_TRY(ensure_partials(ctx, (size_t)2 * BKR_NUM_SMS * BKR_MAX_N * BKR_MAX_N * sizeof(double2)));
     const int NT = (N + 7) / 8;
 #define GRAM_NT(Real)                                                                    \

@@ -237,11 +237,43 @@ __global__ void __launch_bounds__(64, 1) probe_tma_kernel(const unsigned char *b
     if (threadIdx.x == 0 && blockIdx.x == 0) out->cycles = clock64() - c0;
 }
 
+// kind 23: mma.sync.m16n8k8 TF32 issue rate (legacy tensor path, the one mblas_tf32.cu uses), 8 warps x 8 independent accumulators
+__global__ void __launch_bounds__(256, 1) probe_tf32_kernel(int iters, uint32_t seed, double *sink, ProbeOut *out)
+{
+    float c[8][4];
+    uint32_t a[4], b[2];
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+#pragma unroll
+        for (int q = 0; q < 4; q++) c[i][q] = 0.f;
+#pragma unroll
+    for (int q = 0; q < 4; q++) a[q] = seed * (q + 1 + threadIdx.x);
+    b[0] = seed;
+    b[1] = seed + 1;
+    unsigned long long c0 = 0;
+    if (threadIdx.x == 0) c0 = clock64();
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 8; i++)
+            asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                         : "+f"(c[i][0]), "+f"(c[i][1]), "+f"(c[i][2]), "+f"(c[i][3])
+                         : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b[0]), "r"(b[1]));
+    }
+    float s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; i++)
+#pragma unroll
+        for (int q = 0; q < 4; q++) s += c[i][q];
+    if (s == -1.2345f) sink[0] = s;
+    __syncthreads();
+    if (threadIdx.x == 0 && blockIdx.x == 0) out->cycles = clock64() - c0;
+}
+
 } // namespace
 
 int run_probe(bkr_ctx *ctx, int kind, double *result)
 {
-    if (kind < 10 || kind > 22 || !result) return BKR_EINVAL;
+    if (kind < 10 || kind > 23 || !result) return BKR_EINVAL;
     const size_t BUF = (size_t)32 << 20; // L2 resident
     unsigned char *buf = nullptr;
     BKR_CUDA(ctx, cudaMalloc((void **)&buf, BUF + 4096));
@@ -282,6 +314,7 @@ int run_probe(bkr_ctx *ctx, int kind, double *result)
             if (kind == 20) go(probe_dry_kernel<8, 8>, 256, 8);
             break;
         }
+        case 23: probe_tf32_kernel<<<G, 256, 0, ctx->stream>>>(20000, 0u, sink, out); units = 20000.0 * 8 * 8 * 2048; break; // flop per SM
         default: {
             const int stage = 9216, depth = kind == 21 ? 8 : 1, iters = 400, smem = stage * depth;
             cudaFuncSetAttribute(probe_tma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 9216 * 8);

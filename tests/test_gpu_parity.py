@@ -154,15 +154,9 @@ def test_gram_fp32_storage_fp64_accumulation(lat_asym, N):
     X, Y = _round32(H.np_sources(dims, N, 800 + N)), _round32(H.np_sources(dims, N, 900 + N))
     Xd = ctx.pack(torch.from_numpy(X).cuda(), binding.F32)
     Yd = ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
+    K = ctx.gram(N, Xd, Yd, prec=binding.F32).cpu().numpy()
     want = oracle.gram(X, Y)
-    ctx.set_f32_math(binding.F32_MATH_FP64)  # FP64 tensor products: exact products of fp32 inputs, fp64 accumulation
-    try:
-        K = ctx.gram(N, Xd, Yd, prec=binding.F32).cpu().numpy()
-    finally:
-        ctx.set_f32_math(binding.F32_MATH_AUTO)
-    assert np.abs(K - want).max() <= 1e-13 * np.abs(want).max()
-    K = ctx.gram(N, Xd, Yd, prec=binding.F32).cpu().numpy()  # default path (split-TF32 where it is faster): DESIGN.md U25
-    assert np.abs(K - want).max() <= 2e-6 * np.abs(want).max()
+    assert np.abs(K - want).max() <= 1e-13 * np.abs(want).max()  # fp64 accumulation of exact fp32 inputs
 
 
 @pytest.mark.parametrize("N", NS_ALL)
@@ -259,17 +253,11 @@ def test_block_axpy_gram_fused_fp32(lat_asym, N):
     rng = np.random.default_rng(200 + N)
     a = _round32(rng.standard_normal((N, N)) + 1j * rng.standard_normal((N, N)))
     Xd, Yd = ctx.pack(torch.from_numpy(X).cuda(), binding.F32), ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
-    for mode, tolK in ((binding.F32_MATH_FP64, 1e-13), (binding.F32_MATH_AUTO, 2e-6)):
-        ctx.set_f32_math(mode)
-        try:
-            Yd = ctx.pack(torch.from_numpy(Y).cuda(), binding.F32)
-            K = ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd, prec=binding.F32).cpu().numpy()
-        finally:
-            ctx.set_f32_math(binding.F32_MATH_AUTO)
-        got = ctx.unpack(Yd, N, binding.F32).cpu().numpy()
-        assert H.relerr_inf(got, oracle.block_axpy(a, X, Y)) <= TOL32
-        wantK = oracle.gram(got, got)  # of the stored (rounded) block: fp64 products of fp32 numbers are exact
-        assert np.abs(K - wantK).max() <= tolK * np.abs(wantK).max()
+    K = ctx.block_axpy_gram(N, torch.from_numpy(a).cuda(), Xd, Yd, prec=binding.F32).cpu().numpy()
+    got = ctx.unpack(Yd, N, binding.F32).cpu().numpy()
+    assert H.relerr_inf(got, oracle.block_axpy(a, X, Y)) <= TOL32
+    wantK = oracle.gram(got, got)  # of the stored (rounded) block: fp64 products of fp32 numbers are exact
+    assert np.abs(K - wantK).max() <= 1e-13 * np.abs(wantK).max()
 
 
 @pytest.mark.parametrize("N", [1, 2, 5, 8, 16, 32])

@@ -4,7 +4,7 @@ against the oracle's plain fp64 loops (eq. 3 / eq. 4) on the same fp32-
 Error budget: a split product drops x_lo y_lo and truncates the low parts, ~2^-21 per product; a
 reduction keeps fp32 partial sums over 64 rows and fp64 beyond.  Measured 1e-7 .. 7e-7 of the largest entry; asserted
 <= 2e-6 for reductions and <= 1e-5 (the fp32 storage tolerance of the other tests) for updates.  The FP64 tensor path
-(F32_MATH_FP64) stays exact to 1e-13 on the same inputs and is checked beside it.
+(F32_MATH_FP64, the default: exact to 1e-13 on the same inputs) is what the other test files check.
 """
 import numpy as np
 import pytest
@@ -52,7 +52,7 @@ def _tf32(ctx):
             ctx.set_f32_math(binding.F32_MATH_TF32)
 
         def __exit__(self, *a):
-            ctx.set_f32_math(binding.F32_MATH_AUTO)
+            ctx.set_f32_math(binding.F32_MATH_FP64)
     return _Mode()
 
 
@@ -157,9 +157,11 @@ def test_fused_qpx_update_split_tf32(lat, lat_ragged, lat_wrap, N):
         assert H.relerr_inf(ctx.unpack(Xd, N).cpu().numpy(), oracle.block_axpy(Wm, P, X)) <= TOL_GRAM
 
 
-def test_mixed_solver_same_iterations_on_both_tensor_paths(lat_wrap):
-    """the fp32-inner blockCGrQ (Alg. 3) with split-TF32 multi-BLAS against the same solve with exact FP64 tensor products:
-    both reach the tolerance (true residual recomputed by the oracle), iteration counts within 2 %"""
+def test_mixed_solver_converges_on_both_tensor_paths(lat_wrap):
+    """the fp32-inner blockCGrQ (Alg. 3) with split-TF32 multi-BLAS and with exact FP64 tensor products: both reach the
+    tolerance (true residual recomputed by the oracle).  The TF32 path may need more iterations (its products carry
+    ~3e-7 instead of 6e-8: +22 % at config 3, profiles/r2_ncu_summary.md section 6), which is why it is not the default;
+    here only a loose bound is asserted."""
     from paper_1710_09745_b200 import binding
     dims, ctx = lat_wrap
     fat, lng = H.np_links(dims, "random", seed=53)
@@ -167,13 +169,13 @@ def test_mixed_solver_same_iterations_on_both_tensor_paths(lat_wrap):
     B = H.np_sources(dims, N, 6100)
     Bd = torch.from_numpy(B).cuda()
     out = {}
-    for mode in (binding.F32_MATH_FP64, binding.F32_MATH_AUTO):
+    for mode in (binding.F32_MATH_FP64, binding.F32_MATH_TF32):
         ctx.set_f32_math(mode)
         try:
             X, rr, st = ctx.solve_block(0.05, Bd, tol=1e-10, inner_prec=binding.F32, delta=0.1)
         finally:
-            ctx.set_f32_math(binding.F32_MATH_AUTO)
+            ctx.set_f32_math(binding.F32_MATH_FP64)
         assert st["status"] == 0
         assert oracle.true_relres(dims, fat, lng, 0.05, B, X.cpu().numpy()).max() <= 1e-10
         out[mode] = st["iters"]
-    assert abs(out[binding.F32_MATH_AUTO] - out[binding.F32_MATH_FP64]) <= max(2, 0.02 * out[binding.F32_MATH_FP64])
+    assert out[binding.F32_MATH_TF32] <= 1.5 * out[binding.F32_MATH_FP64]
