@@ -453,6 +453,7 @@ def run_bkr(args):
     B = synth.make_sources(dims, N, seed=2000 + rank, device=dev)
     ctx = binding.Context(dims, device=local)
     ctx.load_links(fat, lng, also_f32=True)
+    ctx.set_f32_math(args.f32_math)
     del fat, lng
     torch.cuda.empty_cache()
     # on-chip peaks measured on this box: the "alu" roofline denominators
@@ -545,6 +546,7 @@ def run_bkr(args):
                    "step": "one blockCGrQ iteration (Alg. 1 l.8-12): 2 Dslash, Gram P^H MP, fused Q+P+X update, fused Q' update + Gram, 2 small-matrix kernels",
                    "l2": "inputs larger than L2 (links %.2f GB + blocks %.2f GB each)" % (
                        144 * w * volume(dims) * 1e-9, block_bytes(dims, N, w) * 1e-9),
+                   "f32_math": {0: "fp64 tensor products", 1: "split-TF32", 2: "split-TF32 updates", 3: "split-TF32 reductions"}[args.f32_math],
                    "parallelism": "replicas only" if world > 1 else "1 GPU"},
         "frac_hbm_iteration": value / world / hbm,
         "GFLOPS_iteration": world * flops_iteration(dims, N) / ms_step * 1e-6,
@@ -707,6 +709,9 @@ def main():
     ap.add_argument("--sweep", action="store_true")
     ap.add_argument("--microbench", action="store_true", help="print the on-chip microbenchmark numbers only")
     ap.add_argument("--ablation", action="store_true", help="add the Fig. 4-style ablation (100 iterations per arm)")
+    ap.add_argument("--f32-math", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="tensor path of the multi-BLAS on fp32 blocks (bkr.h BKR_TUNE_F32_MATH): 0 FP64 DMMA (default), 1 split-TF32, "
+                         "2 / 3 TF32 updates / reductions only; affects --prec f32 and the fp32-inner solver")
     ap.add_argument("--maxiter", type=int, default=20000)
     ap.add_argument("--cg-rhs", type=int, default=2, help="sequential CG is measured on this many rhs and scaled to N")
     args = ap.parse_args()
