@@ -1,11 +1,12 @@
 // Multi-BLAS for fp32 blocks on the TF32 tensor path (PAPER.md:245-299 for the operations).
 //
 // mblas.cu widens fp32 operands and contracts them with FP64 DMMA, whose 37 TFLOP/s bind at N >= 16 when the data are
-// only 8 bytes per complex number.  Here every real product is split as (PAPERS.md: the "3xTF32" error-corrected scheme)
-//     x = x_hi + x_lo,   x_hi = x rounded to TF32 (11 significant bits),   x_lo = x - x_hi rounded to TF32,
+// only 8 bytes per complex number.  Here every real product is split as (the "3xTF32" error-corrected scheme)
+//     x = x_hi + x_lo,   x_hi = x rounded to TF32 (11 significant bits),   x_lo = x - x_hi truncated to TF32 by the tensor core,
 //     x y ~= x_lo y_hi + x_hi y_lo + x_hi y_hi                              (x_lo y_lo ~ 2^-22 |x y| dropped)
 // and issued as three mma.sync.m16n8k8 TF32 instructions with fp32 accumulators (measured 280 TFLOP/s = 93 TFLOP/s of
-// split products: profiles/r2_onchip_probes.md section 6).  Partial sums stay in fp32 only over short runs: an update has
+// split products: bkr_microbench kind 23, profiles/r2_onchip_probes.md section 6).  NOT the default: its ~3e-7 errors cost
+// the fp32-inner solver 22 % more iterations at config 3 (mblas.cuh); BKR_TUNE_F32_MATH selects it.  Partial sums stay in fp32 only over short runs: an update has
 // <= 64 terms per output and rounds to fp32 anyway; a reduction adds its fp32 accumulators into fp64 ones every
 // TF_FLUSH k-steps (64 rows), so the long sum over the lattice is fp64 as in mblas.cu.  Error against the fp64
 // product of the same fp32 inputs: <= ~1e-6 relative to the largest entry (tests/test_gpu_tf32.py), against 6e-8 of
