@@ -663,6 +663,7 @@ def run_many(args):
     fat, lng = synth.make_links(dims, kind, seed=1000, device="cuda")
     ctx = binding.Context(dims)
     ctx.load_links(fat, lng, also_f32=True)
+    ctx.set_f32_math(args.f32_math)
     del fat, lng
     nrhs = args.many_rhs
     B = synth.make_sources(dims, nrhs, seed=2000, device="cuda")

@@ -125,9 +125,9 @@ static inline Ring3 plan_ring3(size_t L, int N, size_t fixed, int esize_p)
 // fp32 blocks: FP64 DMMA path of mblas.cu (default) or the split-TF32 tensor path of mblas_tf32.cu.  BKR_TUNE_F32_MATH:
 // 0 = FP64 DMMA (products of fp32 numbers exact, every sum fp64, one rounding on store), 1 = split-TF32 wherever it exists,
 // 2 = split-TF32 updates only, 3 = split-TF32 reductions only.  TF32 is faster per call (32^4, N = 16: update 0.168 -> 0.117 ms,
-// fused update + Gram 0.227 -> 0.184, Gram 0.108 -> 0.098) but its ~3e-7 errors cost the fp32-inner blockCGrQ 22 % more
-// iterations at config 3 (541 -> 657-670 with either the updates or the reductions on TF32), so the solver stays on FP64
-// tensor products.
+// fused update + Gram 0.227 -> 0.184, Gram 0.108 -> 0.098) but its ~3e-7 errors cost the fp32-inner blockCGrQ 25-30 %
+// more iterations at config 3, tol 1e-10 (529 -> 663-686 with either the updates or the reductions on TF32), so the solver
+// stays on FP64 tensor products.
 static inline bool f32_tf32_update(const bkr_ctx *ctx) { const int m = ctx->tune[BKR_TUNE_F32_MATH]; return m == 1 || m == 2; }
 static inline bool f32_tf32_gram(const bkr_ctx *ctx) { const int m = ctx->tune[BKR_TUNE_F32_MATH]; return m == 1 || m == 3; }
 int launch_block_update_tf32(bkr_ctx *ctx, int N, const double2 *a, const void *C, const void *W, void *Z, const int *done, int tri);

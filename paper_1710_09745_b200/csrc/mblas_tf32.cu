@@ -5,13 +5,15 @@
 //     x = x_hi + x_lo,   x_hi = x rounded to TF32 (11 significant bits),   x_lo = x - x_hi truncated to TF32 by the tensor core,
 //     x y ~= x_lo y_hi + x_hi y_lo + x_hi y_hi                              (x_lo y_lo ~ 2^-22 |x y| dropped)
 // and issued as three mma.sync.m16n8k8 TF32 instructions with fp32 accumulators (measured 280 TFLOP/s = 93 TFLOP/s of
-// split products: bkr_microbench kind 23, profiles/r2_onchip_probes.md section 6).  NOT the default: its ~3e-7 errors cost
-// the fp32-inner solver 22 % more iterations at config 3 (mblas.cuh); BKR_TUNE_F32_MATH selects it.  Partial sums stay in fp32 only over short runs: an update has
-// <= 64 terms per output and rounds to fp32 anyway; a reduction adds its fp32 accumulators into fp64 ones every
-// TF_FLUSH k-steps (64 rows), so the long sum over the lattice is fp64 as in mblas.cu.  Error against the fp64
-// product of the same fp32 inputs: <= ~1e-6 relative to the largest entry (tests/test_gpu_tf32.py), against 6e-8 of
-// input rounding.  The rings, the TMA producer warp, the chunk strides, the fixed-order two-stage reduction and the
-// partials layout are those of mblas.cu, so launch_gram_finish / small_kernel take the result unchanged.
+// split products: bkr_microbench kind 23, profiles/r2_onchip_probes.md section 6).  NOT the default: its ~3e-7 errors
+// cost the fp32-inner solver 25-30 % more iterations at config 3, tol 1e-10 (mblas.cuh);
+// BKR_TUNE_F32_MATH selects it.
+// Partial sums stay in fp32 only over short runs: an update has <= 64 terms per output and rounds to fp32 anyway; a
+// reduction adds its fp32 accumulators into fp64 ones every TF_FLUSH k-steps (64 rows), so the long sum over the lattice
+// is fp64 as in mblas.cu.  Error against the fp64 product of the same fp32 inputs: <= ~1e-6 relative to the largest entry
+// (tests/test_gpu_tf32.py), against 6e-8 of input rounding.  The rings, the TMA producer warp, the chunk strides, the
+// fixed-order two-stage reduction and the partials layout are those of mblas.cu, so launch_gram_finish / small_kernel
+// take the result unchanged.
 //
 // Fragments of mma.m16n8k8 (g = lane / 4, t = lane % 4):
 //   A (16 x 8):  a0 = A[g][t]   a1 = A[g + 8][t]   a2 = A[g][t + 4]   a3 = A[g + 8][t + 4]

@@ -160,7 +160,7 @@ def test_fused_qpx_update_split_tf32(lat, lat_ragged, lat_wrap, N):
 def test_mixed_solver_converges_on_both_tensor_paths(lat_wrap):
     """the fp32-inner blockCGrQ (Alg. 3) with split-TF32 multi-BLAS and with exact FP64 tensor products: both reach the
     tolerance (true residual recomputed by the oracle).  The TF32 path may need more iterations (its products carry
-    ~3e-7 instead of 6e-8: +22 % at config 3, profiles/r2_ncu_summary.md section 6), which is why it is not the default;
+    ~3e-7 instead of 6e-8: +25-30 % at config 3, profiles/r2_ncu_summary.md section 4b), which is why it is not the default;
     here only a loose bound is asserted."""
     from paper_1710_09745_b200 import binding
     dims, ctx = lat_wrap
