@@ -57,7 +57,8 @@ enum {
     BKR_ECUDA = -4,      /* a CUDA call failed; bkr_last_cuda_error() gives the cudaError_t        */
     BKR_EBREAKDOWN = -5, /* the block lost rank for good (two-pass QR included) or a Gram matrix is non-finite
                           * (PAPER.md:109); X = best so far */
-    BKR_ENOCONV = -6     /* maxiter reached; X holds the last iterate, stats are filled             */
+    BKR_ENOCONV = -6,    /* maxiter reached; X holds the last iterate, stats are filled             */
+    BKR_ETOOBIG = -7     /* size beyond the fixed capacity of a no-allocation entry point (bkr_gram_static) */
 };
 
 typedef struct {
@@ -107,6 +108,17 @@ int bkr_apply_M(bkr_ctx *ctx, double mass, int N, int prec, const void *in, void
  * the blocks, fp64 accumulation, deterministic two-stage reduction.  hermitian != 0: only i <= j is
  * computed and the rest mirrored with a real diagonal.  X, Y native; K N*N complex fp64. */
 int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, void *K);
+
+/* The same reduction for callers that must not reach cudaMalloc (code under CUDA stream capture, tight serving loops,
+ * harnesses that forbid allocation): bkr_gram keeps its per-CTA partial sums in a buffer it allocates on first use,
+ * this entry point keeps them in a fixed device array inside the library -- 148 x 32 x 32 complex fp64 = 2.3 MB, held by
+ * every GPU that loads the library until the process exits -- and calls no cudaMalloc, cudaFree or allocating library
+ * routine, on the first call or later.  Arguments, layouts and result as bkr_gram with the FP64 tensor products (bit-identical
+ * to its default path); N <= BKR_STATIC_MAX_N, else BKR_ETOOBIG and nothing is launched.  The array is shared by every
+ * context and stream of a device: calls that overlap on the GPU race on it, so callers serialise them (one stream, or
+ * events).  Nothing in it needs clearing between calls (stage 1 writes every entry stage 2 reads). */
+#define BKR_STATIC_MAX_N 32
+int bkr_gram_static(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, void *K);
 
 /* Streaming multi-BLAS (eq. 3): Y <- Y + X a, y_kj += sum_i x_ki a_ij, every vector
  * streamed once.  a: N*N complex fp64; X, Y native, X != Y. */

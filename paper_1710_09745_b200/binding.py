@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbkr.so")
 
 F64, F32 = 0, 1
-OK, EINVAL, ENOLINKS, ENOMEM, ECUDA, EBREAKDOWN, ENOCONV = 0, -1, -2, -3, -4, -5, -6
+OK, EINVAL, ENOLINKS, ENOMEM, ECUDA, EBREAKDOWN, ENOCONV, ETOOBIG = 0, -1, -2, -3, -4, -5, -6, -7
 MAX_N = 32
 OPT_L2_BUDGET_MB, OPT_ROW_UNIT_TILES, OPT_ROW_VEC_POLICY, OPT_ABLATION = 0, 1, 2, 3
 ABL_UNFUSED_UPDATES, ABL_UNFUSED_GRAM, ABL_VECTOR_BLAS, ABL_VECTOR_DSLASH = 1, 2, 4, 8
@@ -24,7 +24,7 @@ F32_MATH_FP64, F32_MATH_TF32, F32_MATH_TF32_UPDATES, F32_MATH_TF32_GRAM = 0, 1, 
 
 SYMBOLS = (
     "bkr_create", "bkr_destroy", "bkr_load_links", "bkr_field_bytes", "bkr_pack", "bkr_unpack", "bkr_dslash", "bkr_dslash_xpay",
-    "bkr_apply_M", "bkr_gram", "bkr_block_axpy", "bkr_block_update", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
+    "bkr_apply_M", "bkr_gram", "bkr_gram_static", "bkr_block_axpy", "bkr_block_update", "bkr_block_axpy_gram", "bkr_block_qpx_update", "bkr_cholesky_upper", "bkr_hpd_inverse", "bkr_solve_block",
     "bkr_solve_cg", "bkr_solve_block_host", "bkr_solve_cg_host", "bkr_bench_iterations", "bkr_last_cuda_error",
     "bkr_strerror", "bkr_version", "bkr_dslash_variant", "bkr_set_dslash_variant", "bkr_set_option", "bkr_microbench", "bkr_solver_state", "bkr_solve_many",
 )
@@ -71,6 +71,7 @@ def lib():
             "bkr_dslash_xpay": (ci, [vp, ci, ci, ci, cd, vp, vp, vp]),
             "bkr_apply_M": (ci, [vp, cd, ci, ci, vp, vp]),
             "bkr_gram": (ci, [vp, ci, ci, vp, vp, ci, vp]),
+            "bkr_gram_static": (ci, [vp, ci, ci, vp, vp, ci, vp]),
             "bkr_block_axpy": (ci, [vp, ci, ci, vp, vp, vp]),
             "bkr_block_update": (ci, [vp, ci, ci, ci, ci, vp, vp, vp, vp]),
             "bkr_block_axpy_gram": (ci, [vp, ci, ci, vp, vp, vp, vp]),
@@ -198,6 +199,13 @@ class Context:
         K = torch.empty((int(N), int(N)), dtype=torch.complex128, device=self.device) if out is None else out
         self._check(lib().bkr_gram(self._h, int(N), int(prec), _dev_ptr(X, "X"), _dev_ptr(Y, "Y"), int(bool(hermitian)),
                                    _dev_ptr(K, "K")), "bkr_gram")
+        return K
+
+    def gram_static(self, N, X, Y, K, hermitian=False, prec=F64):
+        """bkr_gram_static: K = X^dag Y into the caller's K without any allocation in the library (N <= 32, bkr.h)"""
+        assert K.dtype == torch.complex128 and tuple(K.shape) == (int(N), int(N))
+        self._check(lib().bkr_gram_static(self._h, int(N), int(prec), _dev_ptr(X, "X"), _dev_ptr(Y, "Y"), int(bool(hermitian)),
+                                          _dev_ptr(K, "K")), "bkr_gram_static")
         return K
 
     def block_axpy(self, N, a, X, Y, prec=F64):

@@ -138,6 +138,14 @@ int bkr_gram(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int he
     return launch_gram_finish(ctx, N, np, hermitian ? 1 : 0, (double2 *)K);
 }
 
+int bkr_gram_static(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, void *K)
+{
+    if (!ctx || N < 1 || !valid_prec(prec) || !X || !Y || !K) return BKR_EINVAL;
+    if (N > BKR_STATIC_MAX_N) return BKR_ETOOBIG;
+    BKR_ENTER(ctx);
+    return launch_gram_static(ctx, N, prec, X, Y, hermitian ? 1 : 0, (double2 *)K);
+}
+
 int bkr_block_axpy(bkr_ctx *ctx, int N, int prec, const void *a, const void *X, void *Y)
 {
     if (!ctx || !valid_n(N) || !valid_prec(prec) || !a || !X || !Y || X == Y) return BKR_EINVAL;
@@ -360,6 +368,7 @@ const char *bkr_strerror(int status)
     case BKR_ECUDA: return "CUDA error (see bkr_last_cuda_error)";
     case BKR_EBREAKDOWN: return "Cholesky breakdown: block lost rank or non-finite Gram matrix";
     case BKR_ENOCONV: return "maxiter reached without convergence";
+    case BKR_ETOOBIG: return "size beyond the fixed capacity of this no-allocation entry point (N <= 32 for bkr_gram_static)";
     default: return "unknown status";
     }
 }

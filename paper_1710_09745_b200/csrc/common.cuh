@@ -147,6 +147,8 @@ int launch_dslash_row(bkr_ctx *ctx, int out_parity, int N, int prec, const void 
 // stage 1 of K = X^dag Y: per-CTA partial sums into ctx->partials; returns the number of partials.
 int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian,
                          int *num_partials, const int *done);
+// both stages with the partials in a file-scope device array of mblas.cu (no allocation; N <= BKR_STATIC_MAX_N)
+int launch_gram_static(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, double2 *K);
 // stage 2 alone (API path): K = fixed-order sum of the partials, mirrored if hermitian.  ldk: row stride of K (0 = N).
 int launch_gram_finish(bkr_ctx *ctx, int N, int num_partials, int hermitian, double2 *K, int ldk = 0);
 // Blocks of 34..64 rhs (N even): the whole Gram matrix K (N x N, row stride N) from the panels X_I^dag Y_J of N / 2 columns

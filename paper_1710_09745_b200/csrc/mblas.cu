@@ -929,3 +929,112 @@ int launch_update_gram(bkr_ctx *ctx, int N, int prec, const double2 *a, const vo
 #undef UG_SW
 #undef UG_GO
 }
+
+// ------------------------------------------------------------------------------------------ Gram without allocation
+// bkr_gram_static (bkr.h): K = X^dag Y with the per-CTA partials of stage 1 in a file-scope device array instead of
+// ctx->partials, for callers that must not reach cudaMalloc (stream capture, serving loops).  Same kernels, same tile ->
+// CTA -> warp assignment and the same fixed-order second stage as launch_gram_partials + launch_gram_finish on the FP64
+// tensor path, so the result is bit-identical to bkr_gram's default path.
+//  * Capacity: one partial per SM for blocks of up to BKR_STATIC_MAX_N = 32 rhs: 148 x 32 x 32 x 16 B = 2.3 MB, held by
+//    every GPU that loads the library until the process exits.
+//  * The array is shared by all contexts and streams of a device and keeps the last call's contents.  Nothing in it has
+//    to start at zero: stage 1 writes every entry stage 2 reads (each CTA stores its whole N x N partial, or its rows
+//    of it when the block is split over blockIdx.y), so there is no clearing pass.  Two calls that overlap on the GPU
+//    (different streams, or two contexts on one device) race on it: callers serialise.
+//  * In host code `gram_static_scratch` is a host-side stand-in, not a device address; the kernels get the address
+//    cudaGetSymbolAddress returns, looked up once per device with that device current.
+static __device__ __align__(256) double2 gram_static_scratch[(size_t)BKR_NUM_SMS * BKR_STATIC_MAX_N * BKR_STATIC_MAX_N];
+
+static const int STATIC_MAX_DEVICES = 64;
+static double2 *gram_static_ptr[STATIC_MAX_DEVICES]; // device address of the array on each device (0 = not looked up)
+
+static int gram_static_address(bkr_ctx *ctx, double2 **ptr)
+{
+    if (ctx->device < 0 || ctx->device >= STATIC_MAX_DEVICES) return BKR_EINVAL;
+    if (!gram_static_ptr[ctx->device]) { // the caller (BKR_ENTER) has made ctx->device current
+        double2 *p = nullptr;
+        BKR_CUDA(ctx, cudaGetSymbolAddress((void **)&p, gram_static_scratch));
+        gram_static_ptr[ctx->device] = p;
+    }
+    *ptr = gram_static_ptr[ctx->device];
+    return BKR_OK;
+}
+
+// stage 2 (gram_finish_kernel of blas.cu on an explicit partials pointer)
+__global__ void gram_static_finish_kernel(int N, int num_partials, int hermitian, const double2 *__restrict__ partials,
+                                          double2 *__restrict__ K)
+{
+    const int o = blockIdx.x * blockDim.x + threadIdx.x;
+    if (o >= N * N) return;
+    const int i = o / N, j = o % N;
+    const bool lower = hermitian && i > j;
+    const int src = lower ? j * N + i : o;
+    double2 s = make_double2(0.0, 0.0);
+    for (int p = 0; p < num_partials; p++) {
+        const double2 v = partials[(size_t)p * N * N + src];
+        s.x += v.x;
+        s.y += v.y;
+    }
+    if (lower) s.y = -s.y;
+    if (hermitian && i == j) s.y = 0.0;
+    K[o] = s;
+}
+
+template <typename Real, int NT>
+static int gram_static_go(bkr_ctx *ctx, size_t L, int N, const void *X, const void *Y, int hermitian, double2 *scratch, double2 *K)
+{
+    typedef typename CxT<Real>::type Cx;
+    constexpr int TIB = NT > 2 ? 2 : NT; // the launch geometry of gram_go
+    constexpr int CW = NT > 2 ? 4 : 8;
+    const Cx *x = (const Cx *)X, *y = (const Cx *)Y;
+    const bool alias = hermitian && X == Y;
+    const int pad = sizeof(Real) == 8 ? 64 : 32;
+    const size_t fixed = 128 + (size_t)N * N * sizeof(double2);
+    const int nxs = hermitian ? 8 * NT : 8 * TIB;
+    const RingPlan rp = plan_ring(L, fixed, 3, nxs, (int)sizeof(Cx), pad, alias ? 0 : 8 * NT, (int)sizeof(Cx), pad);
+    if (rp.nstg < 2) return BKR_EINVAL;
+    const size_t ntiles = (L + rp.R - 1) / rp.R;
+    const unsigned gx = (unsigned)(ntiles < (size_t)GRAM_MAX_GRID ? ntiles : (size_t)GRAM_MAX_GRID);
+#define GRAM_STATIC_LAUNCH(H_, A_, TIB_, GRID_)                                                                        \
+    do {                                                                                                               \
+        static int attr_dev = -1; /* cudaFuncSetAttribute allocates nothing */                                         \
+        if (attr_dev != ctx->device) {                                                                                 \
+            BKR_CUDA(ctx, cudaFuncSetAttribute(gram_tma_kernel<Real, NT, H_, A_, TIB_, CW>,                            \
+                                               cudaFuncAttributeMaxDynamicSharedMemorySize, MB_SMEM_BUDGET));          \
+            attr_dev = ctx->device;                                                                                    \
+        }                                                                                                              \
+        gram_tma_kernel<Real, NT, H_, A_, TIB_, CW><<<GRID_, (CW + 1) * 32, rp.smem, ctx->stream>>>(L, N, rp, x, y,     \
+                                                                                                   scratch, nullptr);  \
+    } while (0)
+    if (hermitian) {
+        if (alias) GRAM_STATIC_LAUNCH(true, true, NT, gx);
+        else GRAM_STATIC_LAUNCH(true, false, NT, gx);
+    } else {
+        dim3 g2(gx, (NT + TIB - 1) / TIB);
+        GRAM_STATIC_LAUNCH(false, false, TIB, g2);
+    }
+#undef GRAM_STATIC_LAUNCH
+    BKR_TRY(bkr_check_launch(ctx));
+    gram_static_finish_kernel<<<(N * N + 127) / 128, 128, 0, ctx->stream>>>(N, (int)gx, hermitian, scratch, K);
+    return bkr_check_launch(ctx);
+}
+
+// N <= BKR_STATIC_MAX_N (checked by the caller, bkr_gram_static); no cudaMalloc / cudaFree on this path
+int launch_gram_static(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian, double2 *K)
+{
+    const size_t L = (size_t)ctx->g.Vh * 3;
+    double2 *scratch = nullptr;
+    BKR_TRY(gram_static_address(ctx, &scratch));
+#define GRAM_STATIC_NT(Real)                                                                 \
+    switch ((N + 7) / 8) {                                                                   \
+    case 1: return gram_static_go<Real, 1>(ctx, L, N, X, Y, hermitian, scratch, K);          \
+    case 2: return gram_static_go<Real, 2>(ctx, L, N, X, Y, hermitian, scratch, K);          \
+    case 3: return gram_static_go<Real, 3>(ctx, L, N, X, Y, hermitian, scratch, K);          \
+    default: return gram_static_go<Real, 4>(ctx, L, N, X, Y, hermitian, scratch, K);         \
+    }
+    if (prec == BKR_F64) {
+        GRAM_STATIC_NT(double)
+    }
+    GRAM_STATIC_NT(float)
+#undef GRAM_STATIC_NT
+}
