@@ -1,9 +1,11 @@
 // Small dense N x N algebra on the device (PAPER.md:178 does it on the host with Eigen; north_star moves it
 // into a device-side kernel so that no Gram matrix or coefficient matrix ever crosses to the host).
 //
-// One CTA.  All threads: the deterministic second stage of the Gram reduction (fixed-order sum of the per-CTA
-// partials, Hermitised from the upper triangle) and the N x N products.  Warp 0 alone: the
-// Cholesky factorisation H = R^dag R (Algorithm 2 l.3) and the triangular inverse, matrices in shared memory.
+// A cluster of SMALL_CLUSTER CTAs of 1024 threads.  All of them: the deterministic second stage of the Gram reduction
+// (fixed-order sum of the per-CTA partials, Hermitised from the upper triangle), each a slice of the matrix,
+// stored into rank 0's shared memory.  Rank 0 alone: the Cholesky factorisation H = R^dag R (Algorithm 2 l.3), the
+// triangular inverse and the N x N products, matrices in shared memory; up to 32 rhs a thread per matrix element with the
+// element in a register and one barrier per column (16 us per call at N = 16; 43 us before, 57 us in round 1).
 //
 // Modes (Algorithm 1 / 2 / 3 line numbers as reconstructed in DESIGN.md U7):
 //   SMALL_CHOL    API: R = chol(in), Rinv
@@ -18,7 +20,11 @@
 //                 C = R2 R1; Sinv = R2^-1; then as SMALL_INIT
 #include "common.cuh"
 
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
+
 #define SMALL_THREADS 1024
+#define SMALL_CLUSTER 8 /* CTAs that share the second stage of the Gram reduction (load_hermitian); rank 0 does the rest */
 #define SMALL_SMEM4_MAX_N 56 /* 4 x 56^2 x 16 = 196 KB of shared memory; 3 x 64^2 x 16 = 192 KB */
 
 __device__ __forceinline__ double2 cmul(double2 a, double2 b)
@@ -30,22 +36,96 @@ __device__ __forceinline__ double2 cmulc(double2 a, double2 b) // conj(a) * b
     return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
 }
 
-// In-place upper Cholesky of the Hermitian matrix whose upper triangle is in A (row-major, shared memory).
-// On return A = R (upper triangular, real positive diagonal, zeros below).  Whole CTA, right-looking: per column j one
-// pivot test, the scaling of row j and the rank-1 update of the trailing triangle spread over all threads, three
-// barriers (round 1 did this in one warp, a column per lane: 57 us per call at N = 16, most of it dependent
-// shared-memory round trips).  Per element the operations and their order are those of the column version.
+// Named barrier 1 over the first nth threads of the CTA (nth a multiple of 32): the factorisation and the triangular
+// inverse run on 32 x clamp(N, 8, 32) threads -- a barrier over all 32 warps costs twice one over 8.
+__device__ __forceinline__ void bar_part(int nth) { asm volatile("bar.sync 1, %0;" ::"r"(nth) : "memory"); }
+__device__ __forceinline__ int small_part_threads(int N) { return 32 * (N < 8 ? 8 : N > 32 ? 32 : N); }
+
+// N <= 32: thread (warp i, lane c) of the 1024 owns matrix element (i, c) and keeps it in a register; one CTA barrier per
+// column.  A single warp issues one dependent instruction every ~5 cycles, so what counts is the number of instructions on
+// the chain from one pivot to the next, not their latencies (measured on this GPU: DFMA 8, shuffle 9, 1/x 81, rsqrt 74,
+// a 1024-thread barrier 76 cycles): here the chain is a row store, the barrier, three shared-memory reads, a reciprocal
+// and one complex multiply-add, ~220 cycles per column.  Versions tried before it, at N = 16: one warp through shared
+// memory 57 us (round 1); CTA-wide with three barriers and two divisions per column 27 k cycles; one barrier and a warp per
+// trailing row 16 k; one warp with the pivot row in shuffles 32 k (a warp alone is issue bound); this one 3.5 k.
+//
+// Column j: warp j stores its (final, still unscaled) row into R; after the barrier every thread below it subtracts
+// conj(a_ji) a_jc / d, d = a_jj.  At the end row i is scaled by rsqrt(d_i).  Pivot tests as in part_cholesky_upper.
+// Called by ALL threads (the return value is the same in each); the caller puts a barrier behind it.
+__device__ bool reg_cholesky_upper(int N, const double2 *A, double2 *R, double rel_tol, double abs_tol, bool *finite_out, double *h0)
+{
+    const int i = threadIdx.x >> 5, c = threadIdx.x & 31;
+    const bool own = i < N && c < N && c >= i;
+    double2 v = own ? A[i * N + c] : make_double2(0.0, 0.0);
+    if (own && i == c) h0[i] = v.x;
+    *finite_out = true;
+    for (int j = 0; j < N; j++) {
+        if (i == j && c < N) R[j * N + c] = v; // zeros left of the diagonal
+        __syncthreads();
+        const double d = R[j * N + j].x, hjj = h0[j];
+        if (!isfinite(d) || !isfinite(hjj)) {
+            *finite_out = false;
+            return false;
+        }
+        if (!(d > rel_tol * hjj) || !(d > abs_tol)) return false;
+        if (own && i > j) {
+            const double dinv = 1.0 / d;
+            const double2 t = cmulc(R[j * N + i], R[j * N + c]);
+            v.x -= t.x * dinv;
+            v.y -= t.y * dinv;
+        }
+    }
+    __syncthreads(); // the last pivot has been read by everyone
+    if (i < N) { // every row is in R and nobody reads another warp's row any more: scale row i in place
+        const double di = R[i * N + i].x, rin = rsqrt(di);
+        __syncwarp();
+        if (c < N && c >= i) R[i * N + c] = c == i ? make_double2(di * rin, 0.0) : make_double2(v.x * rin, v.y * rin);
+    }
+    return true;
+}
+
+// Ri = R^-1 for N <= 32 in the same layout: thread (i, c) accumulates s_ic = sum_{k > i} R_ik X_kc in a register while the
+// rows of X = R^-1 become final from the bottom up (row k = (e_k - s_k) / R_kk), one CTA barrier per row.  Called by all
+// threads; Ri is complete and visible when it returns.
+__device__ void reg_upper_inverse(int N, const double2 *R, double2 *Ri)
+{
+    const int i = threadIdx.x >> 5, c = threadIdx.x & 31;
+    const bool own = i < N && c < N && c >= i;
+    const double rinv = i < N ? 1.0 / R[i * N + i].x : 0.0;
+    double2 s = make_double2(0.0, 0.0);
+    for (int k = N - 1; k >= 0; k--) {
+        if (i == k && c < N)
+            Ri[k * N + c] = c > k ? make_double2(-s.x * rinv, -s.y * rinv) : c == k ? make_double2(rinv, 0.0) : make_double2(0.0, 0.0);
+        __syncthreads();
+        if (own && i < k && c >= k) {
+            const double2 t = cmul(R[i * N + k], Ri[k * N + c]);
+            s.x += t.x;
+            s.y += t.y;
+        }
+    }
+}
+
+// Upper Cholesky factor of the Hermitian matrix in A (row-major, shared memory; upper triangle read, trailing part
+// overwritten): R (upper triangular, real positive diagonal, zeros below) goes to a second matrix, so that a column step
+// needs ONE barrier: everyone reads the pivot d and the still unscaled row j, writes r_jc = a_jc / sqrt(d) to R and updates
+// the trailing triangle with conj(a_ji) a_jc / d (= conj(r_ji) r_jc).  A warp per trailing row, lanes across its columns.
+// Round 1 did this in one warp through shared memory (57 us at N = 16); the first CTA-wide version took three barriers over
+// 1024 threads and two dependent fp64 divisions per column (27 k cycles at N = 16); this one ~7 k.
+// Called by threads 0 .. nth - 1 only.
 //
 // Breakdown (U15): a pivot that is non-finite, non-positive, or has lost more than 13
 // digits against the diagonal entry it started from (d <= 1e-13 h_jj: the column is linearly dependent on the
 // previous ones to working precision, and only rounding noise decides the sign of the pivot).
 // rel_tol / abs_tol: a pivot must exceed rel_tol * h_jj and abs_tol.  *finite_out: no NaN / Inf was met.  The return
-// value and *finite_out are the same in every thread (they depend on shared-memory values read after a barrier).
-__device__ bool cta_cholesky_upper(int N, double2 *A, double rel_tol, double abs_tol, bool *finite_out, double *h0)
+// value and *finite_out are the same in every calling thread (shared-memory values read after a barrier).
+__device__ bool part_cholesky_upper(int N, double2 *A, double2 *R, double rel_tol, double abs_tol, bool *finite_out, double *h0,
+                                    int nth)
 {
-    const int tid = threadIdx.x, nt = blockDim.x;
-    for (int c = tid; c < N; c += nt) h0[c] = A[c * N + c].x;
-    __syncthreads();
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = nth >> 5;
+    for (int c = tid; c < N; c += nth) h0[c] = A[c * N + c].x;
+    for (int i = 1 + warp; i < N; i += nwarp)
+        for (int c = lane; c < i; c += 32) R[i * N + c] = make_double2(0.0, 0.0);
+    bar_part(nth);
     *finite_out = true;
     for (int j = 0; j < N; j++) {
         const double d = A[j * N + j].x, hjj = h0[j];
@@ -54,114 +134,123 @@ __device__ bool cta_cholesky_upper(int N, double2 *A, double rel_tol, double abs
             return false;
         }
         if (!(d > rel_tol * hjj) || !(d > abs_tol)) return false;
-        const double rjj = sqrt(d);
-        __syncthreads(); // everyone has read the pivot
-        for (int c = tid; c < N; c += nt) {
-            if (c == j) A[j * N + j] = make_double2(rjj, 0.0);
-            else if (c > j) {
-                double2 v = A[j * N + c];
-                A[j * N + c] = make_double2(v.x / rjj, v.y / rjj);
-            } else A[j * N + c] = make_double2(0.0, 0.0);
+        const double rjj = sqrt(d), rinv = 1.0 / rjj, dinv = 1.0 / d;
+        for (int c = j + tid; c < N; c += nth) {
+            const double2 v = A[j * N + c];
+            R[j * N + c] = c == j ? make_double2(rjj, 0.0) : make_double2(v.x * rinv, v.y * rinv);
         }
-        __syncthreads();
-        const int m = N - j - 1; // trailing block: rows / columns j + 1 .. N - 1, upper triangle
-        for (int o = tid; o < m * m; o += nt) {
-            const int i = j + 1 + o / m, c = j + 1 + o % m;
-            if (c < i) continue;
-            const double2 t = cmulc(A[j * N + i], A[j * N + c]);
-            const double2 v = A[i * N + c];
-            A[i * N + c] = make_double2(v.x - t.x, v.y - t.y);
+        for (int i = j + 1 + warp; i < N; i += nwarp) { // trailing block, upper triangle
+            const double2 aji = A[j * N + i];
+            for (int c = i + lane; c < N; c += 32) {
+                const double2 t = cmulc(aji, A[j * N + c]);
+                const double2 v = A[i * N + c];
+                A[i * N + c] = make_double2(v.x - t.x * dinv, v.y - t.y * dinv);
+            }
         }
-        __syncthreads();
+        bar_part(nth);
     }
     return true;
 }
 
-// Ri = R^-1 for upper-triangular R with real diagonal, whole CTA: the entries at distance d = c - i from the diagonal
-// depend only on those at smaller distances, so each distance is one parallel step (a dot product of length d per entry,
-// summed in the order of the column-wise back substitution).
+// Ri = R^-1 for upper-triangular R with real diagonal, 32 < N <= 64, whole CTA, no barrier inside: a warp per column c of Ri,
+// which is the back substitution R x = e_c.  Lane k keeps the running sums s_k = sum_{m > k} R_km x_m of rows k and k + 32;
+// x_i = -s_i / R_ii is formed in the lane that owns row i, broadcast by a shuffle, and every lane above adds R_ki x_i.  The
+// chain per entry is a multiply, a shuffle and a multiply-add.  Called by all threads; ends with a CTA barrier.
 __device__ void cta_upper_inverse(int N, const double2 *R, double2 *Ri)
 {
-    const int tid = threadIdx.x, nt = blockDim.x;
-    for (int o = tid; o < N * N; o += nt) {
-        const int i = o / N, c = o % N;
-        if (i > c) Ri[o] = make_double2(0.0, 0.0);
-        else if (i == c) Ri[o] = make_double2(1.0 / R[o].x, 0.0);
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const double rinv0 = lane < N ? 1.0 / R[lane * N + lane].x : 0.0;
+    const double rinv1 = lane + 32 < N ? 1.0 / R[(lane + 32) * N + lane + 32].x : 0.0;
+    for (int c = warp; c < N; c += nwarp) {
+        double2 s0 = make_double2(0.0, 0.0), s1 = make_double2(0.0, 0.0);
+        for (int i = c; i >= 0; i--) {
+            const bool hi = i >= 32;
+            const double2 s = hi ? s1 : s0;
+            const double ri = hi ? rinv1 : rinv0;
+            double2 xi = i == c ? make_double2(ri, 0.0) : make_double2(-s.x * ri, -s.y * ri);
+            xi.x = __shfl_sync(full, xi.x, i & 31);
+            xi.y = __shfl_sync(full, xi.y, i & 31);
+            if (lane < i) {
+                const double2 t = cmul(R[lane * N + i], xi);
+                s0.x += t.x;
+                s0.y += t.y;
+            }
+            if (lane + 32 < i) {
+                const double2 t = cmul(R[(lane + 32) * N + i], xi);
+                s1.x += t.x;
+                s1.y += t.y;
+            }
+            if (lane == (i & 31)) Ri[i * N + c] = xi;
+        }
+        for (int i = c + 1 + lane; i < N; i += 32) Ri[i * N + c] = make_double2(0.0, 0.0);
     }
     __syncthreads();
-    for (int d = 1; d < N; d++) {
-        for (int i = tid; i + d < N; i += nt) {
-            const int c = i + d;
-            double2 s = make_double2(0.0, 0.0);
-            for (int k = i + 1; k <= c; k++) {
-                double2 t = cmul(R[i * N + k], Ri[k * N + c]);
-                s.x += t.x;
-                s.y += t.y;
-            }
-            const double dd = R[i * N + i].x;
-            Ri[i * N + c] = make_double2(-s.x / dd, -s.y / dd);
-        }
-        __syncthreads();
-    }
 }
 
-__device__ void load_hermitian(const SmallArgs &p, double2 *A)
+__device__ void upper_inverse(int N, const double2 *R, double2 *Ri)
 {
-    const int N = p.N;
+    if (N <= 32) reg_upper_inverse(N, R, Ri);
+    else cta_upper_inverse(N, R, Ri);
+}
+
+// H (N x N, into A0 = the A matrix of cluster rank 0, through distributed shared memory for the other ranks) = the
+// fixed-order sum of the per-CTA partials of the Gram reduction, Hermitised from the upper triangle, or the
+// caller's matrix `in`.  The partials are 148 x N^2 x 16 bytes (0.6 MB at N = 16, 2.4 MB at N = 32): one SM pulls them from
+// L2 at ~20 B/clk, which was 30 k of the kernel's 82 k cycles at N = 16 and 110 k of 240 k at N = 32.  So the kernel runs as
+// a cluster of SMALL_CLUSTER CTAs: rank r sums a contiguous slice of the matrix elements and stores them into rank 0's shared
+// memory; after a cluster barrier rank 0 goes on alone.  Per element, fixed order hence deterministic (P12): 16 lanes take the
+// partials q = g, g + 16, g + 32, ... (all loads of a lane in flight at once), a butterfly over the 16 lanes adds them up; two
+// adjacent elements per warp so that every load instruction reads whole 32-byte sectors.
+__device__ void load_hermitian(const SmallArgs &p, double2 *A0, int rank, int nrank)
+{
+    const int N = p.N, NN = N * N;
     if (p.num_partials > 0) {
-        // Second stage of the Gram reduction, fixed order, hence deterministic (P12): the partials q = 0, 1, 2, ... go to
-        // four running sums by q mod 4, combined as (s0 + s1) + (s2 + s3).  Four adjacent lanes hold the four sums of
-        // one matrix element (eight loads in flight each) and meet through shuffles: one serial chain of ~148 dependent
-        // L2 loads cost 54 us per call, four interleaved chains in one thread ~10 us.
-        const int g = threadIdx.x & 3, lane = threadIdx.x & 31, per = blockDim.x >> 2;
-        const size_t stride = (size_t)N * N;
-        for (int o0 = 0; o0 < N * N; o0 += per) {
-            const int o = o0 + (threadIdx.x >> 2);
-            const bool act = o < N * N;
+        const int per = ((NN + nrank - 1) / nrank + 1) & ~1; // elements per rank, even
+        const int o_lo = rank * per, o_hi = min(NN, o_lo + per);
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+        const int g = lane >> 1, e = lane & 1;
+        const size_t stride = (size_t)NN;
+        for (int ob = o_lo + 2 * warp; ob < o_hi; ob += 2 * nwarp) { // warp-uniform
+            const int o = ob + e;
+            const bool act = o < o_hi;
             const int i = act ? o / N : 0, j = act ? o % N : 0;
             const int src = i <= j ? i * N + j : j * N + i;
             double2 acc = make_double2(0.0, 0.0);
-            if (act) {
-                const double2 *pp = p.partials + src;
-                int q = g;
-                for (; q + 28 < p.num_partials; q += 32) {
-                    double2 v[8];
+            const double2 *pp = p.partials + src;
+            for (int q0 = g; q0 < p.num_partials; q0 += 160) {
+                double2 v[10];
 #pragma unroll
-                    for (int c = 0; c < 8; c++) v[c] = pp[(size_t)(q + 4 * c) * stride];
-#pragma unroll
-                    for (int c = 0; c < 8; c++) {
-                        acc.x += v[c].x;
-                        acc.y += v[c].y;
-                    }
+                for (int c = 0; c < 10; c++) {
+                    const int q = q0 + 16 * c;
+                    v[c] = (act && q < p.num_partials) ? pp[(size_t)q * stride] : make_double2(0.0, 0.0);
                 }
-                for (; q < p.num_partials; q += 4) {
-                    const double2 v = pp[(size_t)q * stride];
-                    acc.x += v.x;
-                    acc.y += v.y;
+#pragma unroll
+                for (int c = 0; c < 10; c++) {
+                    acc.x += v[c].x;
+                    acc.y += v[c].y;
                 }
             }
-            const int b0 = lane & ~3;
-            const double x0 = __shfl_sync(0xffffffffu, acc.x, b0), x1 = __shfl_sync(0xffffffffu, acc.x, b0 + 1),
-                         x2 = __shfl_sync(0xffffffffu, acc.x, b0 + 2), x3 = __shfl_sync(0xffffffffu, acc.x, b0 + 3);
-            const double y0 = __shfl_sync(0xffffffffu, acc.y, b0), y1 = __shfl_sync(0xffffffffu, acc.y, b0 + 1),
-                         y2 = __shfl_sync(0xffffffffu, acc.y, b0 + 2), y3 = __shfl_sync(0xffffffffu, acc.y, b0 + 3);
+#pragma unroll
+            for (int m = 2; m <= 16; m <<= 1) {
+                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, m);
+                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, m);
+            }
             if (act && g == 0) {
-                double2 s = make_double2((x0 + x1) + (x2 + x3), (y0 + y1) + (y2 + y3));
-                if (i > j) s.y = -s.y;
-                if (i == j) s.y = 0.0;
-                A[o] = s;
+                if (i > j) acc.y = -acc.y;
+                if (i == j) acc.y = 0.0;
+                A0[o] = acc;
             }
         }
-    } else {
-        for (int o = threadIdx.x; o < N * N; o += blockDim.x) {
+    } else if (rank == 0) {
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) {
             const int i = o / N, j = o % N;
             double2 s = p.in[i <= j ? o : j * N + i];
             if (i > j) s.y = -s.y;
             if (i == j) s.y = 0.0;
-            A[o] = s;
+            A0[o] = s;
         }
     }
-    __syncthreads();
 }
 
 // residual norms from C (PAPER.md:208 with the index fix U11): r_i = ||C[:,i]|| / ||b_i||
@@ -182,8 +271,10 @@ __device__ double max_relres(int N, const double2 *C, const double *bnorm2, doub
     return m;
 }
 
-__global__ void __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
+__global__ void __cluster_dims__(SMALL_CLUSTER, 1, 1) __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
 {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int rank = (int)cluster.block_rank();
     extern __shared__ double2 sm[];
     const int N = p.N, NN = N * N;
     // four N x N matrices; above N = 56 the fourth (a read-mostly copy) lives in global memory: 4 x 64^2 x 16 bytes do not fit
@@ -191,15 +282,18 @@ __global__ void __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
     __shared__ int ok_s, finite_s;
     __shared__ double scratch[BKR_MAX_N], h0s[BKR_MAX_N];
     SolverFlags *fl = p.flags;
-    if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) {
-        if (p.mode == SMALL_BETA && threadIdx.x == 0) { // no new W: nothing left to apply to X after this iteration
+    if (p.mode >= SMALL_BETA && p.mode <= SMALL_QR && fl->done) { // the same in every CTA of the cluster
+        if (p.mode == SMALL_BETA && threadIdx.x == 0 && rank == 0) { // no new W: nothing left to apply to X after this iteration
             fl->xpend = 0;
             fl->xidle = 1;
         }
         return;
     }
 
-    load_hermitian(p, A);
+    cluster.sync(); // every CTA of the cluster runs: its shared memory may be written from the others
+    load_hermitian(p, cluster.map_shared_rank(A, 0), rank, SMALL_CLUSTER);
+    cluster.sync();
+    if (rank != 0) return;
     if (p.mode == SMALL_RQ1) { // shifted Cholesky QR: H + s 1, s = 1e-12 max_i H_ii
         double hmax = 0.0;
         for (int i = 0; i < N; i++) hmax = fmax(hmax, A[i * N + i].x);
@@ -207,19 +301,30 @@ __global__ void __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
         if (threadIdx.x < N) A[threadIdx.x * N + threadIdx.x].x += 1e-12 * hmax;
         __syncthreads();
     }
+    const int nth = small_part_threads(N);
     {
         // Breakdown thresholds (U15): 13 digits lost against the diagonal entry for Gram matrices of fp64 blocks;
         // fp32 blocks carry rounding noise of ~1e-7 h_jj, so a rank-deficient one would pass that test with a noise pivot:
         // the caller passes pivot_tol = 4e-6 there.  Pass 2 of the two-pass QR: columns have norm <= 1 after pass 1, a
         // pivot below 1e-8 is the image of rounding noise (no full rank).
         const double rel = p.pivot_tol > 0.0 ? p.pivot_tol : 1e-13;
-        bool fin = true;
-        bool ok = cta_cholesky_upper(N, A, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin, h0s); // A = R
-        if (ok) cta_upper_inverse(N, A, B); // B = R^-1
+        bool fin = true, okc = true;
+        if (N <= 32) {
+            okc = reg_cholesky_upper(N, A, Cm, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin, h0s); // Cm = R
+        } else if ((int)threadIdx.x < nth) {
+            okc = part_cholesky_upper(N, A, Cm, rel, p.mode == SMALL_RQ2 ? 1e-8 : 0.0, &fin, h0s, nth);
+        }
         if (threadIdx.x == 0) {
-            ok_s = ok ? 1 : 0;
+            ok_s = okc ? 1 : 0;
             finite_s = fin ? 1 : 0;
         }
+    }
+    __syncthreads();
+    if (ok_s) upper_inverse(N, Cm, B); // B = R^-1 (uniform branch; complete and visible on return)
+    {
+        double2 *t = A; // from here on A = R; the matrix the factorisation worked in is scratch
+        A = Cm;
+        Cm = t;
     }
     __syncthreads();
     const bool ok = ok_s != 0;
@@ -249,12 +354,15 @@ __global__ void __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
         break;
     case SMALL_HPDINV:
     case SMALL_BETA: {
-        // beta = R^-1 R^-dag : beta_ij = sum_k Ri_ik conj(Ri_jk), k >= max(i,j)
+        // beta = R^-1 R^-dag : beta_ij = sum_k Ri_ik conj(Ri_jk), k >= max(i,j).  The lanes of a warp run over j: Ri_jk is read
+        // from a transposed copy (in A: R is not needed any more), else every lane hits the same bank (21 k cycles at N = 32)
+        for (int o = threadIdx.x; o < NN; o += blockDim.x) A[(o % N) * N + o / N] = B[o];
+        __syncthreads();
         for (int o = threadIdx.x; o < NN; o += blockDim.x) {
             int i = o / N, j = o % N;
             double2 s = make_double2(0.0, 0.0);
             for (int k = (i > j ? i : j); k < N; k++) {
-                double2 t = cmulc(B[j * N + k], B[i * N + k]);
+                double2 t = cmulc(A[k * N + j], B[i * N + k]);
                 s.x += t.x;
                 s.y += t.y;
             }
@@ -364,7 +472,7 @@ __global__ void __launch_bounds__(SMALL_THREADS) small_kernel(SmallArgs p)
         // A = C_new, B = C_new^-1.  S = C_new Cprev^-1 (Alg. 3 l.6, C_old = C before this iteration's l.12: U12)
         for (int o = threadIdx.x; o < NN; o += blockDim.x) Dm[o] = p.Cprev[o];
         __syncthreads();
-        cta_upper_inverse(N, Dm, Cm); // Cm = Cprev^-1
+        upper_inverse(N, Dm, Cm); // Cm = Cprev^-1
         for (int o = threadIdx.x; o < NN; o += blockDim.x) {
             int i = o / N, j = o % N;
             double2 s = make_double2(0.0, 0.0);
@@ -407,7 +515,7 @@ int launch_small(bkr_ctx *ctx, const SmallArgs &args_in)
                              (int)(4 * SMALL_SMEM4_MAX_N * SMALL_SMEM4_MAX_N * sizeof(double2)));
         attr_dev = ctx->device;
     }
-    small_kernel<<<1, SMALL_THREADS, smem, ctx->stream>>>(args);
+    small_kernel<<<SMALL_CLUSTER, SMALL_THREADS, smem, ctx->stream>>>(args); // one cluster (__cluster_dims__)
     return bkr_check_launch(ctx);
 }
 
