@@ -143,6 +143,35 @@ int launch_dslash_win(bkr_ctx *ctx, int out_parity, int N, int prec, const void 
 int launch_dslash_row(bkr_ctx *ctx, int out_parity, int N, int prec, const void *in, void *out, const void *xp,
                       double a, const int *done);
 
+// Second stage of the Gram reduction for one matrix element, by 16 lanes of a warp (lane bits 1..4 = g): the sum of
+// pp[q * stride], q = 0 .. np - 1, where lane g adds q = g, g + 16, g + 32, ... (all its loads in flight at once) and a
+// butterfly over the 16 lanes adds the 16 sums -- a fixed order, so every caller (small_kernel, gram_finish_kernel,
+// bkr_gram_static) gets bit-identical results from the same partials (P12).  Whole warps must call it; act = this lane's
+// element exists.  Lane bit 0 distinguishes two elements handled by one warp.
+__device__ __forceinline__ double2 sum_partials_16(const double2 *pp, size_t stride, int np, int g, bool act)
+{
+    double2 acc = make_double2(0.0, 0.0);
+    for (int q0 = g; q0 < np; q0 += 160) {
+        double2 v[10];
+#pragma unroll
+        for (int c = 0; c < 10; c++) {
+            const int q = q0 + 16 * c;
+            v[c] = (act && q < np) ? pp[(size_t)q * stride] : make_double2(0.0, 0.0);
+        }
+#pragma unroll
+        for (int c = 0; c < 10; c++) {
+            acc.x += v[c].x;
+            acc.y += v[c].y;
+        }
+    }
+#pragma unroll
+    for (int m = 2; m <= 16; m <<= 1) {
+        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, m);
+        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, m);
+    }
+    return acc;
+}
+
 // ---- blas.cu
 // stage 1 of K = X^dag Y: per-CTA partial sums into ctx->partials; returns the number of partials.
 int launch_gram_partials(bkr_ctx *ctx, int N, int prec, const void *X, const void *Y, int hermitian,

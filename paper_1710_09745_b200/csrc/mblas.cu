@@ -960,24 +960,22 @@ static int gram_static_address(bkr_ctx *ctx, double2 **ptr)
     return BKR_OK;
 }
 
-// stage 2 (gram_finish_kernel of blas.cu on an explicit partials pointer)
-__global__ void gram_static_finish_kernel(int N, int num_partials, int hermitian, const double2 *__restrict__ partials,
-                                          double2 *__restrict__ K)
+// stage 2 (gram_finish_kernel of blas.cu on an explicit partials pointer: same order of summation)
+__global__ void __launch_bounds__(128)
+gram_static_finish_kernel(int N, int num_partials, int hermitian, const double2 *__restrict__ partials, double2 *__restrict__ K)
 {
-    const int o = blockIdx.x * blockDim.x + threadIdx.x;
-    if (o >= N * N) return;
-    const int i = o / N, j = o % N;
+    const int w = (blockIdx.x * 128 + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int g = lane >> 1, o = 2 * w + (lane & 1);
+    const bool act = o < N * N;
+    const int i = act ? o / N : 0, j = act ? o % N : 0;
     const bool lower = hermitian && i > j;
-    const int src = lower ? j * N + i : o;
-    double2 s = make_double2(0.0, 0.0);
-    for (int p = 0; p < num_partials; p++) {
-        const double2 v = partials[(size_t)p * N * N + src];
-        s.x += v.x;
-        s.y += v.y;
+    const int src = lower ? j * N + i : i * N + j;
+    double2 s = sum_partials_16(partials + src, (size_t)N * N, num_partials, g, act);
+    if (act && g == 0) {
+        if (lower) s.y = -s.y;
+        if (hermitian && i == j) s.y = 0.0;
+        K[o] = s;
     }
-    if (lower) s.y = -s.y;
-    if (hermitian && i == j) s.y = 0.0;
-    K[o] = s;
 }
 
 template <typename Real, int NT>
@@ -1015,7 +1013,7 @@ static int gram_static_go(bkr_ctx *ctx, size_t L, int N, const void *X, const vo
     }
 #undef GRAM_STATIC_LAUNCH
     BKR_TRY(bkr_check_launch(ctx));
-    gram_static_finish_kernel<<<(N * N + 127) / 128, 128, 0, ctx->stream>>>(N, (int)gx, hermitian, scratch, K);
+    gram_static_finish_kernel<<<(N * N * 16 + 127) / 128, 128, 0, ctx->stream>>>(N, (int)gx, hermitian, scratch, K);
     return bkr_check_launch(ctx);
 }
 

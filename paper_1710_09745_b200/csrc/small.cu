@@ -216,26 +216,7 @@ __device__ void load_hermitian(const SmallArgs &p, double2 *A0, int rank, int nr
             const bool act = o < o_hi;
             const int i = act ? o / N : 0, j = act ? o % N : 0;
             const int src = i <= j ? i * N + j : j * N + i;
-            double2 acc = make_double2(0.0, 0.0);
-            const double2 *pp = p.partials + src;
-            for (int q0 = g; q0 < p.num_partials; q0 += 160) {
-                double2 v[10];
-#pragma unroll
-                for (int c = 0; c < 10; c++) {
-                    const int q = q0 + 16 * c;
-                    v[c] = (act && q < p.num_partials) ? pp[(size_t)q * stride] : make_double2(0.0, 0.0);
-                }
-#pragma unroll
-                for (int c = 0; c < 10; c++) {
-                    acc.x += v[c].x;
-                    acc.y += v[c].y;
-                }
-            }
-#pragma unroll
-            for (int m = 2; m <= 16; m <<= 1) {
-                acc.x += __shfl_xor_sync(0xffffffffu, acc.x, m);
-                acc.y += __shfl_xor_sync(0xffffffffu, acc.y, m);
-            }
+            double2 acc = sum_partials_16(p.partials + src, stride, p.num_partials, g, act);
             if (act && g == 0) {
                 if (i > j) acc.y = -acc.y;
                 if (i == j) acc.y = 0.0;
