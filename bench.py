@@ -210,7 +210,10 @@ PROBE_KINDS = [(10, "lds128_conflict_free_B_per_clk_sm", "bytes"), (11, "lds128_
                (18, "dry_stencil_T4_8warps_dfma_per_clk_sm", "dfma"), (19, "dry_stencil_T8_4warps_dfma_per_clk_sm", "dfma"),
                (20, "dry_stencil_T8_8warps_dfma_per_clk_sm", "dfma"),
                (21, "tma_9KB_issue_interval_clk_one_lane", "interval"), (22, "tma_9KB_round_trip_clk_idle_l2", "interval"),
-               (23, "mma_sync_tf32_m16n8k8_flop_per_clk_sm", "flop")]
+               (23, "mma_sync_tf32_m16n8k8_flop_per_clk_sm", "flop"),
+               (24, "latency_dfma_dependent_clk", "interval"), (25, "latency_fp64_reciprocal_plus_add_clk", "interval"),
+               (26, "latency_fp64_rsqrt_plus_add_clk", "interval"), (27, "latency_shfl64_plus_add_clk", "interval"),
+               (28, "latency_sts_lds_round_trip_clk", "interval"), (29, "latency_syncthreads_1024_clk", "interval")]
 
 
 def run_probes(ctx):

@@ -245,7 +245,7 @@ int bkr_set_option(bkr_ctx *ctx, int option, int value);
 /* Measured on-chip peaks for the rooflines (not on the hot path).  kind: 0 fp64 FMA, 1 fp32 FMA,
  * 2 fp64 tensor MMA (m8n8k4), 3 L2 -> SM bandwidth by 16-byte loads, 4 the same by TMA bulk copies, 5 shared-memory read
  * bandwidth.  Runs `reps` launches on the context's stream, synchronises, and writes result[0] = ms per launch,
- * result[1] = flop (kinds 0-2) or bytes (kinds 3-5) per launch.  Kinds 10-22 are the on-chip probes of csrc/probes.cu
+ * result[1] = flop (kinds 0-2) or bytes (kinds 3-5) per launch.  Kinds 10-29 are the on-chip probes of csrc/probes.cu
  * (register-file / shared-memory / TMA sharing, the stencil's dry loop): result[0] = SM cycles, result[1] = work units per
  * SM, result[2] = a second work count or 0.  result: HOST array of 4 doubles. */
 int bkr_microbench(bkr_ctx *ctx, int kind, int reps, double *result);

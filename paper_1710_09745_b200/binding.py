@@ -348,7 +348,7 @@ class Context:
         return float(r[0]), float(r[1])
 
     def probe(self, kind):
-        """on-chip probe `kind` (10..22, csrc/probes.cu): (SM cycles, work units per SM, second work count)"""
+        """on-chip probe `kind` (10..29, csrc/probes.cu): (SM cycles, work units per SM, second work count)"""
         r = (ctypes.c_double * 4)()
         self._check(lib().bkr_microbench(self._h, int(kind), 1, r), "bkr_microbench")
         return float(r[0]), float(r[1]), float(r[2])

@@ -242,7 +242,7 @@ int launch_cg_scalar(bkr_ctx *ctx, int N, int step, double tol, CgScalars *s, So
 
 // ---- microbench.cu
 int run_microbench(bkr_ctx *ctx, int kind, int reps, double *result);
-// ---- probes.cu (kinds 10..22: result[0] = SM cycles, [1] = work units per SM, [2] = second work count)
+// ---- probes.cu (kinds 10..29: result[0] = SM cycles, [1] = work units per SM, [2] = second work count)
 int run_probe(bkr_ctx *ctx, int kind, double *result);
 
 // ---- solver.cu

@@ -269,11 +269,42 @@ __global__ void __launch_bounds__(256, 1) probe_tf32_kernel(int iters, uint32_t 
     if (threadIdx.x == 0 && blockIdx.x == 0) out->cycles = clock64() - c0;
 }
 
+// kinds 24..29: dependent-chain latencies of one warp (what bounds the small-matrix kernel, small.cu): cycles per operation of a
+// chain of 512 dependent operations, in a 1024-thread CTA whose other warps have exited (24..28) or all take part (29).
+//   24 DFMA   25 1.0 / x (+ add)   26 rsqrt (+ add)   27 64-bit shuffle (+ add)   28 shared-memory store -> load round trip
+//   29 __syncthreads over 1024 threads
+__global__ void __launch_bounds__(1024, 1) probe_latency_kernel(int kind, double seed, double *sink, ProbeOut *out)
+{
+    __shared__ double sm[1024];
+    sm[threadIdx.x] = seed;
+    __syncthreads();
+    if (kind != 29 && threadIdx.x >= 32) return;
+    const int n = 512;
+    double x = seed + threadIdx.x;
+    const unsigned long long c0 = clock64();
+    if (kind == 24) for (int i = 0; i < n; i++) x = fma(x, 1.0000001, 1e-9);
+    if (kind == 25) for (int i = 0; i < n; i++) x = 1.0 / x + 1.5;
+    if (kind == 26) for (int i = 0; i < n; i++) x = rsqrt(x) + 1.5;
+    if (kind == 27) for (int i = 0; i < n; i++) x = __shfl_sync(0xffffffffu, x, (i + 1) & 31) + 1e-9;
+    if (kind == 28) for (int i = 0; i < n; i++) {
+        volatile double *q = &sm[(threadIdx.x + 32 * (i & 15)) & 1023];
+        *q = x;
+        x = *q + 1e-9;
+    }
+    if (kind == 29) for (int i = 0; i < n; i++) {
+        __syncthreads();
+        x += 1e-9;
+    }
+    const unsigned long long c1 = clock64();
+    if (x == -1.2345) sink[0] = x;
+    if (threadIdx.x == 0 && blockIdx.x == 0) out->cycles = c1 - c0;
+}
+
 } // namespace
 
 int run_probe(bkr_ctx *ctx, int kind, double *result)
 {
-    if (kind < 10 || kind > 23 || !result) return BKR_EINVAL;
+    if (kind < 10 || kind > 29 || !result) return BKR_EINVAL;
     const size_t BUF = (size_t)32 << 20; // L2 resident
     unsigned char *buf = nullptr;
     BKR_CUDA(ctx, cudaMalloc((void **)&buf, BUF + 4096));
@@ -314,6 +345,10 @@ int run_probe(bkr_ctx *ctx, int kind, double *result)
             if (kind == 20) go(probe_dry_kernel<8, 8>, 256, 8);
             break;
         }
+        case 24: case 25: case 26: case 27: case 28: case 29:
+            probe_latency_kernel<<<1, 1024, 0, ctx->stream>>>(kind, 1.5, sink, out);
+            units = 512;
+            break;
         case 23: probe_tf32_kernel<<<G, 256, 0, ctx->stream>>>(20000, 0u, sink, out); units = 20000.0 * 8 * 8 * 2048; break; // flop per SM
         default: {
             const int stage = 9216, depth = kind == 21 ? 8 : 1, iters = 400, smem = stage * depth;
