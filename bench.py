@@ -457,6 +457,8 @@ def run_bkr(args):
     ctx = binding.Context(dims, device=local)
     ctx.load_links(fat, lng, also_f32=True)
     ctx.set_f32_math(args.f32_math)
+    for kv in args.tune:
+        ctx.set_option(binding.OPT_TUNE + int(kv.split("=")[0]), int(kv.split("=")[1]))
     del fat, lng
     torch.cuda.empty_cache()
     # on-chip peaks measured on this box: the "alu" roofline denominators
@@ -716,6 +718,8 @@ def main():
     ap.add_argument("--f32-math", type=int, default=0, choices=[0, 1, 2, 3],
                     help="tensor path of the multi-BLAS on fp32 blocks (bkr.h BKR_TUNE_F32_MATH): 0 FP64 DMMA (default), 1 split-TF32, "
                          "2 / 3 TF32 updates / reductions only; affects --prec f32 and the fp32-inner solver")
+    ap.add_argument("--tune", action="append", default=[], metavar="K=V",
+                    help="launch-policy knob BKR_TUNE_K = V (bkr.h), e.g. --tune 5=32 --tune 6=32; repeatable")
     ap.add_argument("--maxiter", type=int, default=20000)
     ap.add_argument("--cg-rhs", type=int, default=2, help="sequential CG is measured on this many rhs and scaled to N")
     args = ap.parse_args()

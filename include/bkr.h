@@ -231,6 +231,8 @@ enum {
     BKR_TUNE_F32_MATH = 4,        /* multi-BLAS on fp32 blocks: 0 = FP64 tensor products, exact (default); 1 = split-TF32   */
                                   /* everywhere it exists (faster per call, ~3e-7 errors: more solver iterations);          */
                                   /* 2 = split-TF32 updates only; 3 = split-TF32 reductions only                            */
+    BKR_TUNE_FUSE_QPX_MAX_N = 5,  /* largest block for which the solver uses the fused Q / P / X update (default 32 = the limit)   */
+    BKR_TUNE_FUSE_GRAM_MAX_N = 6, /* largest block for which it fuses the Q' update with its Gram matrix (default 16, <= 32)   */
     BKR_TUNE_COUNT = 16
 };
 enum {

@@ -665,7 +665,9 @@ static int pqx_go(bkr_ctx *ctx, size_t L, int N, const double2 *Si, const double
                  double2 *X, const SolverFlags *fl)
 {
     typedef typename CxT<RealP>::type CxP;
-    constexpr int CW = 8;
+    // 9 warps get the register budget of 12 (168 per thread); with 3-4 column tiles the fragments and accumulators need more:
+    // 7 consumer warps + the producer = 8 warps = 255 registers per thread, no spills
+    constexpr int CW = NTJ >= 3 ? 7 : 8;
     const size_t fixed = (128 + (size_t)6 * NIS * NTJ * 32 * sizeof(double) + 127) / 128 * 128;
     const Ring3 rp = plan_ring3(L, N, fixed, (int)sizeof(CxP));
     if (rp.nstg < 2) return BKR_EINVAL;
@@ -883,7 +885,7 @@ static int update_gram_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const
                           const int *done)
 {
     typedef typename CxT<Real>::type Cx;
-    constexpr int CW = 8;
+    constexpr int CW = NT >= 3 ? 7 : 8; // 8 warps in all: 255 registers per thread (pqx_go)
     const size_t off_red = (128 + (size_t)2 * NIS * NT * 32 * sizeof(double) + 127) / 128 * 128;
     const size_t fixed = off_red + (size_t)N * N * sizeof(double2);
     const RingPlan rp = plan_ring(L, fixed, 4, N, (int)sizeof(Cx), 32, N, (int)sizeof(Cx), 16);

@@ -225,15 +225,17 @@ __global__ void set_identity_kernel(int N, double2 *A)
     for (int o = threadIdx.x; o < N * N; o += blockDim.x) A[o] = make_double2(o / N == o % N ? 1.0 : 0.0, 0.0);
 }
 
-// Fused Q / P / X update (pqx_update_kernel) only up to 24 rhs: beyond, the update kernels are bound by the FP64 tensor
-// pipe, the fused ones spill, and separate kernels are faster (32^4, N = 32: 5.39 vs 5.58 ms per iteration; N = 24: 3.82
-// vs 3.76 ms).  BKR_ABL_UNFUSED_UPDATES (Fig. 4-style comparison runs) switches it off: five separate passes, X updated
-// right after l.9 as in the unfused Algorithm 1.
-static const int FUSE_MAX_N = 24;
+// Fused Q / P / X update (pqx_update_kernel) up to 32 rhs, the limit of its tiles.  With 3-4 column tiles it runs 7 consumer
+// warps (8 warps in all: 255 registers per thread; with 9 warps ptxas had 168 and spilled, and the fused path lost to separate
+// kernels above 24 rhs).  Measured on 32^4 per iteration, fused / unfused: N = 28 4.76 / 4.87 ms, N = 32 5.04 / 5.21 ms.
+// BKR_TUNE_FUSE_QPX_MAX_N lowers the limit; BKR_ABL_UNFUSED_UPDATES (Fig. 4-style comparison runs) switches the fusion off:
+// five separate passes, X updated right after l.9 as in the unfused Algorithm 1.
+static const int FUSE_MAX_N = 32;
 
 static bool fuse_qpx(const bkr_ctx *ctx, int N)
 {
-    return N <= FUSE_MAX_N && !(ctx->ablation & (BKR_ABL_UNFUSED_UPDATES | BKR_ABL_VECTOR_BLAS));
+    const int nmax = ctx->tune[BKR_TUNE_FUSE_QPX_MAX_N] > 0 ? ctx->tune[BKR_TUNE_FUSE_QPX_MAX_N] : FUSE_MAX_N;
+    return N <= nmax && N <= 32 && !(ctx->ablation & (BKR_ABL_UNFUSED_UPDATES | BKR_ABL_VECTOR_BLAS));
 }
 
 // Alg. 1 l.3-l.6 (and Alg. 3 l.4-l.6 when relupd): R = B - M Xcur in fp64, thin QR, Q in inner precision, P kept.
@@ -326,8 +328,10 @@ static int block_iteration(bkr_ctx *ctx, Workspace *w, double mass, double tol, 
     // l.11 Q S = Q - (M P) beta   (thin QR = Gram + Cholesky + scale, Algorithm 2)
     const bool fuse_gram = !(ctx->ablation & (BKR_ABL_UNFUSED_GRAM | BKR_ABL_VECTOR_BLAS));
     // N <= 16 only: with 3-4 column tiles the reduction's 6-10 tile-pair accumulators no longer fit beside the update's
-    // (ptxas spills; measured 4.08 vs 3.76 ms per iteration at N = 24, 5.76 vs 5.58 at N = 32 on 32^4)
-    if (fuse_gram && N <= 16) { // one pass: Q' and stage 1 of H = Q'^dag Q'
+    // (the fused kernel is bound by its tensor work there: 1.09 ms against 0.48 + 0.28 ms for update + aliased Gram at N = 32 on
+    // 32^4; per iteration 3.86 vs 3.69 ms at N = 24, 5.33 vs 5.04 at N = 32.  BKR_TUNE_FUSE_GRAM_MAX_N raises the limit.)
+    const int gmax = ctx->tune[BKR_TUNE_FUSE_GRAM_MAX_N] > 0 ? ctx->tune[BKR_TUNE_FUSE_GRAM_MAX_N] : 16;
+    if (fuse_gram && N <= gmax && N <= 32) { // one pass: Q' and stage 1 of H = Q'^dag Q'
         BKR_TRY(launch_update_gram(ctx, N, pr, w->negbeta, w->Q, w->AP, w->Q, &np, done));
     } else {
         BKR_TRY(blk_update(ctx, N, pr, pr, w->negbeta, w->Q, w->AP, w->Q, done, 0));
