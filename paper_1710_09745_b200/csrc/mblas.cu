@@ -665,9 +665,10 @@ static int pqx_go(bkr_ctx *ctx, size_t L, int N, const double2 *Si, const double
                  double2 *X, const SolverFlags *fl)
 {
     typedef typename CxT<RealP>::type CxP;
-    // 9 warps get the register budget of 12 (168 per thread); with 3-4 column tiles the fragments and accumulators need more:
-    // 7 consumer warps + the producer = 8 warps = 255 registers per thread, no spills
-    constexpr int CW = NTJ >= 3 ? 7 : 8;
+    // 9 warps get the register budget of 12 (168 per thread); with 4 column tiles the fragments and accumulators need more:
+    // 7 consumer warps + the producer = 8 warps = 255 registers per thread, no spills (32^4, N = 32: 1.50 -> 1.25 ms; with
+    // 3 tiles nothing spills at 168 and 8 warps are faster: 0.78 against 0.79 ms at N = 24)
+    constexpr int CW = NTJ >= 4 ? 7 : 8;
     const size_t fixed = (128 + (size_t)6 * NIS * NTJ * 32 * sizeof(double) + 127) / 128 * 128;
     const Ring3 rp = plan_ring3(L, N, fixed, (int)sizeof(CxP));
     if (rp.nstg < 2) return BKR_EINVAL;
@@ -885,7 +886,8 @@ static int update_gram_go(bkr_ctx *ctx, size_t L, int N, const double2 *a, const
                           const int *done)
 {
     typedef typename CxT<Real>::type Cx;
-    constexpr int CW = NT >= 3 ? 7 : 8; // 8 warps in all: 255 registers per thread (pqx_go)
+    constexpr int CW = 8; // (7 warps at 255 registers end the spills of the 3-4 tile instances but are slower: 0.65 / 1.12 ms
+                          // against 0.55 / 0.83 ms at N = 24 / 32 on 32^4; the solver fuses this pair only up to 16 rhs)
     const size_t off_red = (128 + (size_t)2 * NIS * NT * 32 * sizeof(double) + 127) / 128 * 128;
     const size_t fixed = off_red + (size_t)N * N * sizeof(double2);
     const RingPlan rp = plan_ring(L, fixed, 4, N, (int)sizeof(Cx), 32, N, (int)sizeof(Cx), 16);

@@ -225,7 +225,7 @@ __global__ void set_identity_kernel(int N, double2 *A)
     for (int o = threadIdx.x; o < N * N; o += blockDim.x) A[o] = make_double2(o / N == o % N ? 1.0 : 0.0, 0.0);
 }
 
-// Fused Q / P / X update (pqx_update_kernel) up to 32 rhs, the limit of its tiles.  With 3-4 column tiles it runs 7 consumer
+// Fused Q / P / X update (pqx_update_kernel) up to 32 rhs, the limit of its tiles.  With 4 column tiles it runs 7 consumer
 // warps (8 warps in all: 255 registers per thread; with 9 warps ptxas had 168 and spilled, and the fused path lost to separate
 // kernels above 24 rhs).  Measured on 32^4 per iteration, fused / unfused: N = 28 4.76 / 4.87 ms, N = 32 5.04 / 5.21 ms.
 // BKR_TUNE_FUSE_QPX_MAX_N lowers the limit; BKR_ABL_UNFUSED_UPDATES (Fig. 4-style comparison runs) switches the fusion off:
