@@ -146,7 +146,7 @@ int bkr_block_axpy_gram(bkr_ctx *ctx, int N, int prec, const void *a, const void
 int bkr_block_qpx_update(bkr_ctx *ctx, int N, int prec, const void *Sinv, const void *Sdag, const void *Wm, void *Q,
                          const void *P, void *Pn, void *X, int do_qp, int do_x);
 
-/* Small dense algebra on the device, one warp (Algorithm 2 l.3):
+/* Small dense algebra on the device, one kernel launch (Algorithm 2 l.3):
  * bkr_cholesky_upper: H = R^dag R, R upper triangular with real positive diagonal; Rinv = R^-1.
  * bkr_hpd_inverse   : Ginv = G^-1 for Hermitian positive-definite G (via Cholesky).
  * Inputs use the upper triangle only.  status (device int, may be NULL) receives BKR_OK/BKR_EBREAKDOWN. */
